@@ -1,0 +1,289 @@
+"""T0: pins for the CPU oracle.  No GPU.
+
+Every check here ties oracle/ to something other than itself: the paper's cost
+and update definitions worked by hand (golden fixtures), closed forms, library
+routines (SVD, least squares) on special cases, brute-force NNLS, and invariants
+that a dropped term / wrong index / transposed operand would break.
+"""
+import itertools
+import os
+from fractions import Fraction
+
+import numpy as np
+import pytest
+
+from oracle import nmf_oracle as orc
+from oracle import nmf_numpy as onp
+from paper_2309_04623_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _parse_rows(s):
+    return np.array([[float(Fraction(t)) for t in row.split()] for row in s.split(" / ")])
+
+
+def _load_p4():
+    d = {}
+    for line in open(os.path.join(GOLD, "p4_worked_example.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        key, rest = line.split(None, 1)
+        d[key] = _parse_rows(rest.strip())
+    return d
+
+
+@pytest.fixture(scope="module")
+def tiny():
+    return inputs.make_tiny()
+
+
+# ---- P4: exact-rational worked example -------------------------------------
+def test_p4_worked_example():
+    g = _load_p4()
+    X, Om, W0, H0 = g["X"], g["Omega"], g["W0"], g["H0"]
+    assert orc.objective(X, Om, W0, H0) == pytest.approx(46.0, rel=1e-14)
+    H1 = orc.h_step(X, Om, W0, H0)
+    np.testing.assert_allclose(H1, g["H1"], rtol=1e-14, atol=0)
+    assert orc.objective(X, Om, W0, H1) == pytest.approx(g["f_H1"][0, 0], rel=1e-13)
+    W1 = orc.w_step(X, Om, W0, H1)
+    np.testing.assert_allclose(W1, g["W1"], rtol=1e-13)
+    assert orc.objective(X, Om, W1, H1) == pytest.approx(g["f_W1"][0, 0], rel=2e-9)
+    W2, H2, tr = orc.fit(X, Om, W0, H0, 2, trace=True)
+    np.testing.assert_allclose(tr, [46.0, g["f_H1"][0, 0], g["f_W1"][0, 0], g["f_H2"][0, 0], g["f_W2"][0, 0]],
+                               rtol=2e-9)
+    np.testing.assert_allclose(W2, g["W2"], rtol=2e-9)
+    np.testing.assert_allclose(H2, g["H2"], rtol=2e-9, atol=0)
+    assert np.all(H2[:, 2] == 0.0)     # fully masked column -> exactly 0 (G4)
+
+
+def test_p4b_k1_hand_example():
+    X = np.array([[1.0, 2.0], [3.0, 4.0]])
+    w0 = np.ones((2, 1)); h0 = np.ones((1, 2))
+    for line in open(os.path.join(GOLD, "p4b_k1_example.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        t = line.split()
+        Om = np.ones((2, 2)) if t[0] == "case_full" else np.array([[1.0, 0.0], [1.0, 1.0]])
+        h1 = [float(Fraction(v)) for v in t[2:4]]
+        w1 = [float(Fraction(v)) for v in t[5:7]]
+        f = [float(Fraction(v)) for v in t[8:11]]
+        W, H, tr = orc.fit(X, Om, w0, h0, 1, trace=True)
+        np.testing.assert_allclose(H.ravel(), h1, rtol=1e-15)
+        np.testing.assert_allclose(W.ravel(), w1, rtol=1e-15)
+        np.testing.assert_allclose(tr, f, rtol=1e-13)
+
+
+# ---- P1 + P2: monotone objective on both half-steps, non-negativity ----------
+def test_p1_p2_monotone_nonneg(tiny):
+    p = tiny
+    W, H, tr = orc.fit(p.X, p.Omega, p.W0, p.H0, 200, trace=True)
+    assert np.all(tr[1:] <= tr[:-1] * (1 + 1e-12)), "objective increased on a half-step"
+    assert tr[-1] < 1e-3 * tr[0]
+    assert np.all(W >= 0) and np.all(H >= 0) and np.all(np.isfinite(W)) and np.all(np.isfinite(H))
+    # step-by-step API agrees with the fused loop, and zeros stay zeros
+    W0z = p.W0.astype(np.float64).copy(); W0z[3, 2] = 0.0
+    H0z = p.H0.astype(np.float64).copy(); H0z[1, 100] = 0.0
+    Wz, Hz = orc.fit(p.X, p.Omega, W0z, H0z, 5)
+    assert Wz[3, 2] == 0.0 and Hz[1, 100] == 0.0
+
+
+def test_p1_monotone_weighted_rowvarying():
+    """Heteroscedastic, row-varying zeros (the general Omega of Eq. 2)."""
+    rng = np.random.default_rng(7)
+    N, P, K = 9, 157, 4
+    X = rng.random((N, P)).astype(np.float32) * 10
+    Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.3)).astype(np.float32)
+    W0 = 0.1 + rng.random((N, K)); H0 = 0.1 + rng.random((K, P))
+    _, _, tr = orc.fit(X, Om, W0, H0, 60, trace=True)
+    assert np.all(tr[1:] <= tr[:-1] * (1 + 1e-12))
+
+
+# ---- P3: mask invariance, bitwise ------------------------------------------
+@pytest.mark.parametrize("garbage", [1e30, np.nan, np.inf, -5.0])
+def test_p3_mask_invariance(tiny, garbage):
+    p = tiny
+    W, H = orc.fit(p.X, p.Omega, p.W0, p.H0, 20)
+    Xg = p.X.copy(); Xg[p.Omega == 0] = garbage
+    Wg, Hg = orc.fit(Xg, p.Omega, p.W0, p.H0, 20)
+    assert np.array_equal(W, Wg) and np.array_equal(H, Hg)
+    assert orc.objective(Xg, p.Omega, W, H) == orc.objective(p.X, p.Omega, W, H)
+    Tg = p.T.copy(); Tg[p.omega_t == 0] = garbage
+    assert np.array_equal(orc.project(H, Tg, p.omega_t, p.C0, 10), orc.project(H, p.T, p.omega_t, p.C0, 10))
+
+
+# ---- P5: noise-free rank-K recovery ----------------------------------------
+def test_p5_rank_k_recovery():
+    p = inputs.make_tiny(noise=0.0)
+    norm = float(np.sum(p.Omega.astype(np.float64) * p.X.astype(np.float64) ** 2))
+    _, _, tr = orc.fit(p.X, p.Omega, p.W0, p.H0, 2000, trace=True)
+    assert np.all(tr[1:] <= tr[:-1] * (1 + 1e-12))
+    assert tr[400] / norm <= 1e-3      # after 200 iterations
+    assert tr[-1] / norm <= 1e-5       # after 2000 iterations
+
+
+# ---- P6: fixed point -------------------------------------------------------
+def test_p6_fixed_point():
+    rng = np.random.default_rng(3)
+    N, P, K = 7, 93, 3
+    Ws = 0.2 + rng.random((N, K)); Hs = 0.2 + rng.random((K, P))
+    X = (Ws @ Hs)
+    X32 = X.astype(np.float32)
+    # make X exactly representable so that X == Ws Hs holds for the fp32 input
+    Ws = np.round(Ws * 64) / 64; Hs = np.round(Hs * 64) / 64
+    X32 = (Ws @ Hs).astype(np.float32)
+    assert np.array_equal(X32.astype(np.float64), Ws @ Hs)
+    Om = (rng.random((N, P)) > 0.2).astype(np.float32) * 0.5
+    W, H = orc.fit(X32, Om, Ws, Hs, 100)
+    live = Om.max(axis=0) > 0
+    np.testing.assert_allclose(W, Ws, rtol=1e-12)
+    np.testing.assert_allclose(H[:, live], Hs[:, live], rtol=1e-12)
+
+
+# ---- P7: K=1 closed form + dominant singular pair --------------------------
+def test_p7_k1_closed_form_and_svd():
+    rng = np.random.default_rng(11)
+    N, P = 12, 200
+    X = rng.random((N, P)).astype(np.float32) + 0.05
+    Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.25)).astype(np.float32)
+    w = 0.1 + rng.random((N, 1)); h = 0.1 + rng.random((1, P))
+    Xd, Od = X.astype(np.float64), Om.astype(np.float64)
+    # K=1: the update does not depend on the old value (weighted rank-1 ALS)
+    h1 = orc.h_step(X, Om, w, h)
+    np.testing.assert_allclose(h1[0], (Od * Xd * w).sum(0) / (Od * w * w).sum(0), rtol=1e-12)
+    w1 = orc.w_step(X, Om, w, h1)
+    np.testing.assert_allclose(w1[:, 0], (Od * Xd * h1).sum(1) / (Od * h1 * h1).sum(1), rtol=1e-12)
+    # Omega == 1: converges to the dominant singular pair (Perron-Frobenius)
+    ones = np.ones_like(X)
+    W, H, tr = orc.fit(X, ones, w, h, 60, trace=True)
+    s = np.linalg.svd(Xd, compute_uv=False)
+    assert tr[-1] == pytest.approx((Xd ** 2).sum() - s[0] ** 2, rel=1e-10)
+
+
+# ---- P8: homogeneity, bitwise ----------------------------------------------
+def test_p8_power_of_two_homogeneity(tiny):
+    p = tiny
+    W, H = orc.fit(p.X, p.Omega, p.W0, p.H0, 15)
+    W8, H8 = orc.fit(p.X * np.float32(8), p.Omega, p.W0 * np.float32(8), p.H0, 15)
+    assert np.array_equal(H8, H) and np.array_equal(W8, W * 8)
+    Wo, Ho = orc.fit(p.X, p.Omega * np.float32(0.25), p.W0, p.H0, 15)
+    assert np.array_equal(Ho, H) and np.array_equal(Wo, W)
+
+
+# ---- P9: permutation equivariance ------------------------------------------
+def test_p9_equivariance():
+    rng = np.random.default_rng(5)
+    N, P, K = 8, 120, 4
+    X = rng.random((N, P)).astype(np.float32)
+    Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.2)).astype(np.float32)
+    W0 = 0.1 + rng.random((N, K)); H0 = 0.1 + rng.random((K, P))
+    W, H = orc.fit(X, Om, W0, H0, 12)
+    pn, pp, pk = rng.permutation(N), rng.permutation(P), rng.permutation(K)
+    Wn, Hn = orc.fit(X[pn], Om[pn], W0[pn], H0, 12)
+    np.testing.assert_allclose(Wn, W[pn], rtol=1e-12); np.testing.assert_allclose(Hn, H, rtol=1e-12)
+    Wp, Hp = orc.fit(X[:, pp], Om[:, pp], W0, H0[:, pp], 12)
+    np.testing.assert_allclose(Wp, W, rtol=1e-12); np.testing.assert_allclose(Hp, H[:, pp], rtol=1e-12)
+    Wk, Hk = orc.fit(X, Om, W0[:, pk], H0[pk], 12)
+    np.testing.assert_allclose(Wk, W[:, pk], rtol=1e-12); np.testing.assert_allclose(Hk, H[pk], rtol=1e-12)
+
+
+# ---- P10 + P11: projection = NNLS (brute force) and KKT ---------------------
+def _nnls_bruteforce(Hm, t, om):
+    """min_{c>=0} sum om (t - c H)^2 by enumerating all 2^K supports."""
+    K = Hm.shape[0]
+    sw = np.sqrt(om)
+    A = (Hm * sw).T; b = t * sw
+    best, best_c = np.inf, None
+    for r in range(K + 1):
+        for sup in itertools.combinations(range(K), r):
+            c = np.zeros(K)
+            if sup:
+                sol = np.linalg.lstsq(A[:, sup], b, rcond=None)[0]
+                if np.any(sol < 0):
+                    continue
+                c[list(sup)] = sol
+            f = float(np.sum((A @ c - b) ** 2))
+            if f < best:
+                best, best_c = f, c
+    return best, best_c
+
+
+def test_p10_p11_projection_nnls_kkt(tiny):
+    p = tiny
+    _, H = orc.fit(p.X, p.Omega, p.W0, p.H0, 50)
+    t = p.T[0].astype(np.float64); om = p.omega_t[0].astype(np.float64)
+    f_star, c_star = _nnls_bruteforce(H, t, om)
+    c = orc.project(H, p.T, p.omega_t, p.C0, 3000)[0]
+    f = float(np.sum(om * (t - c @ H) ** 2))
+    assert f == pytest.approx(f_star, rel=1e-10)
+    np.testing.assert_allclose(c, c_star, rtol=1e-6, atol=1e-8 * np.abs(c_star).max())
+    # KKT residual (P11)
+    g = (om * (c @ H - t)) @ H.T
+    active = c <= 1e-9 * c.max()          # MU approaches an active bound geometrically, never exactly
+    kkt = np.where(active, np.minimum(g, 0.0), np.abs(g))
+    assert np.abs(kkt).max() / np.abs((om * t) @ H.T).max() < 1e-9
+    # with an active constraint: a target anti-correlated with one component
+    t2 = np.maximum(t - 3.0 * H[0] * t.max() / H[0].max(), 0).astype(np.float32)[None]
+    f2, c2 = _nnls_bruteforce(H, t2[0].astype(np.float64), om)
+    c2m = orc.project(H, t2, p.omega_t, p.C0, 20000)[0]
+    assert float(np.sum(om * (t2[0] - c2m @ H) ** 2)) == pytest.approx(f2, rel=1e-8)
+
+
+def test_projection_omega_none_and_rows_independent(tiny):
+    p = inputs.make_tiny(M=3)
+    _, H = orc.fit(p.X, p.Omega, p.W0, p.H0, 10)
+    ones = np.ones_like(p.T)
+    assert np.array_equal(orc.project(H, p.T, None, p.C0, 7), orc.project(H, p.T, ones, p.C0, 7))
+    call = orc.project(H, p.T, p.omega_t, p.C0, 7)
+    for m in range(3):
+        assert np.array_equal(call[m:m + 1], orc.project(H, p.T[m:m + 1], p.omega_t[m:m + 1], p.C0[m:m + 1], 7))
+
+
+# ---- P12: two independent oracles -------------------------------------------
+def test_p12_two_oracles_tiny(tiny):
+    p = tiny
+    W, H = orc.fit(p.X, p.Omega, p.W0, p.H0, 200)
+    W2, H2 = onp.fit(p.X, p.Omega, p.W0, p.H0, 200)
+    assert np.linalg.norm(W - W2) / np.linalg.norm(W) < 1e-12
+    assert np.linalg.norm(H - H2) / np.linalg.norm(H) < 1e-12
+    assert orc.objective(p.X, p.Omega, W, H) == pytest.approx(onp.objective(p.X, p.Omega, W, H), rel=1e-12)
+
+
+def test_p12_two_oracles_miri_reduced():
+    p = inputs.make_miri(N=24, S=64, K=8, M=2)
+    W, H = orc.fit(p.X, p.Omega, p.W0, p.H0, 50)
+    W2, H2 = onp.fit(p.X, p.Omega, p.W0, p.H0, 50)
+    assert np.linalg.norm(W - W2) / np.linalg.norm(W) < 1e-12
+    assert np.linalg.norm(H - H2) / np.linalg.norm(H) < 1e-12
+
+
+# ---- subtraction --------------------------------------------------------------
+def test_subtract_definition_and_special_cases():
+    rng = np.random.default_rng(2)
+    M, P, K = 3, 50, 4
+    H = np.round(rng.random((K, P)) * 16); C = np.round(rng.random((M, K)) * 8)
+    T = (C @ H).astype(np.float32)                       # exactly representable model
+    om = (rng.random((M, P)) > 0.3).astype(np.float32)
+    out = orc.subtract(H, T, C, om, None, fill=-7.0)
+    assert np.all(out[om > 0] == 0.0) and np.all(out[om == 0] == -7.0)
+    assert np.array_equal(orc.subtract(H, T, C * 0, None, None), T.astype(np.float64))
+    fac = np.array([0.0, 1.0, 2.0])
+    out = orc.subtract(H, T, C, None, fac)
+    np.testing.assert_array_equal(out, T - fac[:, None] * (C @ H))
+    Tn = T.copy(); Tn[om == 0] = np.nan
+    assert np.all(np.isfinite(orc.subtract(H, Tn, C, om, None, fill=0.0)))
+
+
+# ---- generators: structure facts stated in DESIGN.md / SURVEY §8(d) ----------
+def test_generator_structure():
+    p = inputs.make_tiny()
+    assert p.X.shape == (16, 4096) and p.X.dtype == np.float32 and int((p.Omega[0] == 0).sum()) == 113
+    assert p.W0.min() >= 0.1 and p.W0.max() < 1.0 and p.H0.dtype == np.float32
+    q = inputs.make_miri(N=4, M=1)
+    assert int((q.Omega[0] == 0).sum()) == 1727 and q.X.min() >= 0
+    assert np.array_equal(q.Omega[0] == 0, q.Omega[3] == 0)
+    p2 = inputs.make_tiny()
+    assert np.array_equal(p.X, p2.X) and np.array_equal(p.H0, p2.H0)    # seeded
+    s = inputs.make_stis(N=3, S=128, K=4, M=1)
+    frac = float((s.Omega[0] == 0).mean())
+    assert 0.05 < frac < 0.08
