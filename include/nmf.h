@@ -1,0 +1,155 @@
+/*
+ * nmf.h -- C-ABI boundary of the B200-native weighted-NMF hot path of
+ * arXiv 2309.04623 ("NMF-based GPU accelerated coronagraphy pipeline").
+ *
+ * The library implements, as hand-written sm_100a CUDA kernels, exactly the
+ * steps SURVEY.md section 8(a) lists: component construction by the weighted
+ * multiplicative updates of the paper's Eq. 3 (section 2),
+ * non-negative projection of science frames on the fixed components
+ * ("target modelling") and PSF subtraction.
+ *
+ * Notation (BASELINE.json orientation; the paper writes V for Omega):
+ *   X      [N,P]  reference library, N frames x P pixels, >= 0 where Omega > 0
+ *   Omega  [N,P]  weights; 0 = occulted / bad pixel ("missing data"),
+ *                 else inverse variance (Eq. 2)
+ *   W      [N,K]  coefficients            H [K,P] components
+ * Everything is fp32, row-major, innermost index contiguous.
+ *
+ * General rules for every entry point
+ *   - Pointers named *_dev / documented "device" are CUDA device pointers owned
+ *     by the caller (e.g. torch tensors); pointers documented "host" are plain
+ *     host memory.  The library never frees or keeps a user pointer after the
+ *     call's work has been enqueued, except the workspace set on the plan.
+ *   - Device base pointers must be 16-byte aligned and P % 4 == 0
+ *     (128-bit / TMA loads).  Violations return NMF_ERR_ALIGNMENT.
+ *   - Calls are asynchronous: they enqueue work on the plan's stream and return
+ *     without synchronising, unless stated otherwise (nmf_objective,
+ *     nmf_*_host).  The plan's workspace is used by every call, so calls on one
+ *     plan must be stream-ordered (one stream per plan).
+ *   - Return value: NMF_OK (0) or a negative nmf_status code.  No exceptions and
+ *     no abort cross this boundary.  Asynchronous CUDA faults surface at the next
+ *     call or at nmf_objective / a *_host call.
+ *   - Numerical conventions: entries with Omega == 0 are
+ *     skipped (select semantics; X may hold NaN/Inf there); every ratio is
+ *     num / max(den, 1e-30f); H is updated first, then W with the new H.
+ *   - Preconditions that are documented, not checked: X >= 0 and finite where
+ *     Omega > 0; Omega >= 0; W, H, coef >= 0 on entry (an exact zero stays zero).
+ *   - Results are bitwise reproducible run to run for a fixed plan shape on a
+ *     fixed device (all cross-CTA sums are fixed-order).
+ */
+#ifndef PAPER_2309_04623_NMF_H
+#define PAPER_2309_04623_NMF_H
+
+#include <stddef.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum nmf_status {
+    NMF_OK = 0,
+    NMF_ERR_INVALID_ARG = -1, /* null pointer; N/P/K/M/iters out of range; M > max_targets   */
+    NMF_ERR_ALIGNMENT   = -2, /* base pointer not 16-byte aligned or P % 4 != 0              */
+    NMF_ERR_UNSUPPORTED = -3, /* N > 256 or K > 128 (compiled limits)                        */
+    NMF_ERR_WORKSPACE   = -4, /* workspace missing or smaller than nmf_plan_workspace_bytes  */
+    NMF_ERR_ARCH        = -5, /* current device is not compute capability 10.x               */
+    NMF_ERR_CUDA        = -6  /* CUDA runtime / launch error (sticky until the plan is freed) */
+} nmf_status;
+
+#define NMF_MAX_N 256
+#define NMF_MAX_K 128
+
+typedef struct nmf_plan nmf_plan; /* opaque; owns host-side launch state only */
+
+/* Create a plan for problems of shape (N frames, P pixels, K components).
+ *   batch        >= 1  number of independent problems nmf_fit_batched handles
+ *   max_targets  >= 0  largest M accepted by nmf_project / nmf_subtract
+ * Binds to the CUDA device that is current at the time of the call.
+ * Errors: INVALID_ARG, ALIGNMENT (P % 4), UNSUPPORTED, ARCH, CUDA.            */
+int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int max_targets);
+
+/* Bytes of device scratch the plan needs (split-K partial slabs, objective
+ * partials).  The caller allocates it (16-byte aligned) and hands it over with
+ * nmf_plan_set_workspace; it must stay valid until the plan is destroyed or a
+ * new workspace is set.  Contents need no initialisation.                      */
+size_t nmf_plan_workspace_bytes(const nmf_plan* plan);
+int nmf_plan_set_workspace(nmf_plan* plan, void* workspace_dev, size_t bytes);
+
+/* cudaStream_t to enqueue on, passed as void*.  NULL = the legacy default stream. */
+int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
+
+/* Select the fit kernel family: 0 = automatic (fused per-pixel-tile kernel when
+ * the shape is inside its compiled range, else the generic two-kernel path),
+ * 1 = force generic, 2 = force fused (UNSUPPORTED at fit time if out of range).
+ * Both families compute the same updates; they differ in summation order only.  */
+int nmf_plan_set_variant(nmf_plan* plan, int variant);
+/* Which family nmf_fit will run for this plan: 1 = generic, 2 = fused.            */
+int nmf_plan_get_variant(const nmf_plan* plan);
+
+int nmf_plan_destroy(nmf_plan* plan); /* frees host state and any internal staging buffers */
+
+/* Component construction: `iters` times { H half-step ; W half-step } of Eq. 3
+ * (PAPER.md:48-50), fixed count, no early stop.
+ *   X, Omega  device [N,P]   read-only
+ *   W         device [N,K]   in: initial coefficients, out: result (in place)
+ *   H         device [K,P]   in: initial components,   out: result (in place)
+ * Errors: INVALID_ARG (null, iters < 0), ALIGNMENT, WORKSPACE, CUDA.              */
+int nmf_fit(nmf_plan* plan, const float* X, const float* Omega, float* W, float* H, int iters);
+
+/* The same for `batch` independent problems of identical shape, stored
+ * contiguously: X, Omega [B,N,P]; W [B,N,K]; H [B,K,P].  One launch sequence.     */
+int nmf_fit_batched(nmf_plan* plan, const float* X, const float* Omega, float* W, float* H,
+                    int iters);
+
+/* Target modelling: non-negative projection of M science frames on fixed H by
+ * `iters` W-type updates of Eq. 3, c <- c o (omega o t)H^T / (omega o (cH))H^T,
+ * each frame independently.
+ *   H       device [K,P]  read-only     target device [M,P] read-only
+ *   omega   device [M,P]  read-only, or NULL = all ones
+ *   coef    device [M,K]  in: initial coefficients, out: result (in place)
+ * Errors: INVALID_ARG (M < 1, M > max_targets, ...), ALIGNMENT, WORKSPACE, CUDA.   */
+int nmf_project(nmf_plan* plan, const float* H, const float* target, const float* omega,
+                float* coef, int M, int iters);
+
+/* PSF subtraction: out[m,p] = target[m,p] - factor[m] * sum_k coef[m,k] H[k,p]
+ * (PAPER.md:89, 99).  Where omega is given and omega[m,p] == 0 the output is
+ * `fill` and target[m,p] is not read into the result.
+ *   factor  device [M] or NULL = 1 (slot for best-factor finding)
+ *   out     device [M,P], may not alias the inputs.                                */
+int nmf_subtract(nmf_plan* plan, const float* H, const float* target, const float* coef,
+                 const float* omega, const float* factor, float fill, float* out, int M);
+
+/* Diagnostic: the cost of Eq. 2, sum over Omega>0 of
+ * Omega*(X-WH)^2, accumulated in fp64.  SYNCHRONISES the plan's stream and
+ * writes one double to host memory.                                               */
+int nmf_objective(nmf_plan* plan, const float* X, const float* Omega, const float* W,
+                  const float* H, double* out_host);
+
+/* End-to-end convenience for callers whose data lives in HOST memory: copies
+ * X, Omega, W, H host->device into plan-owned staging buffers (allocated on
+ * first use, freed by nmf_plan_destroy), runs nmf_fit, copies W and H back and
+ * SYNCHRONISES.  All four pointers are host pointers (pinned memory makes the
+ * copies faster but is not required).  W, H are updated in place.                  */
+int nmf_fit_host(nmf_plan* plan, const float* X_host, const float* Omega_host, float* W_host,
+                 float* H_host, int iters);
+
+/* Host-memory end-to-end projection + subtraction of M science frames on
+ * components already resident on the device (H is a DEVICE pointer, e.g. the
+ * result of nmf_fit): copies target/omega/coef in, runs nmf_project and
+ * nmf_subtract (factor = 1), copies coef and the residual images back and
+ * SYNCHRONISES.  omega_host may be NULL.                                           */
+int nmf_project_subtract_host(nmf_plan* plan, const float* H_dev, const float* target_host,
+                              const float* omega_host, float* coef_host, float fill,
+                              float* out_host, int M, int iters);
+
+/* Number of kernel launches this plan has enqueued so far (bench bookkeeping).     */
+long long nmf_plan_launch_count(const nmf_plan* plan);
+
+const char* nmf_status_string(int code);
+/* Text of the last CUDA error recorded on the plan ("" if none).                   */
+const char* nmf_plan_last_cuda_error(const nmf_plan* plan);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* PAPER_2309_04623_NMF_H */

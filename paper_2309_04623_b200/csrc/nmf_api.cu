@@ -1,0 +1,232 @@
+// nmf_api.cu -- the extern "C" boundary declared in include/nmf.h:
+// argument validation, plan/workspace management, dispatch to the kernel families.
+#include "nmf_common.cuh"
+#include <new>
+
+namespace {
+
+inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) & 15u) != 0; }
+
+size_t plan_workspace(nmf_plan* p) {
+    size_t g = nmf_generic_workspace(p);
+    size_t f = nmf_fused_workspace(p);
+    size_t main = nmf_align_up(g > f ? g : f, 256);
+    return main + nmf_align_up(nmf_aux_workspace(p), 256);
+}
+
+int check_ws(const nmf_plan* p) {
+    if (!p->ws || p->ws_bytes < p->ws_needed) return NMF_ERR_WORKSPACE;
+    return NMF_OK;
+}
+
+bool use_fused(const nmf_plan* p) {
+    if (p->variant_req == 1) return false;
+    return nmf_fused_available(p);
+}
+
+int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!X || !Om || !W || !H || iters < 0 || batch < 1 || batch > p->batch) return NMF_ERR_INVALID_ARG;
+    if (misaligned(X) || misaligned(Om) || misaligned(W) || misaligned(H)) return NMF_ERR_ALIGNMENT;
+    int rc = check_ws(p);
+    if (rc) return rc;
+    if (iters == 0) return NMF_OK;
+    if (p->variant_req == 2 && !nmf_fused_available(p)) return NMF_ERR_UNSUPPORTED;
+    if (use_fused(p)) return nmf_fused_fit(p, X, Om, W, H, iters, batch);
+    return nmf_generic_fit(p, X, Om, W, H, iters, batch);
+}
+
+int ensure_stage(nmf_plan* p, size_t bytes) {
+    if (p->stage_bytes >= bytes) return NMF_OK;
+    if (p->stage) { cudaFree(p->stage); p->stage = nullptr; p->stage_bytes = 0; }
+    NMF_CUDA_TRY(p, cudaMalloc(&p->stage, bytes));
+    p->stage_bytes = bytes;
+    return NMF_OK;
+}
+
+int ensure_own_ws(nmf_plan* p) {
+    if (p->ws && p->ws_bytes >= p->ws_needed) return NMF_OK;
+    if (!p->own_ws) NMF_CUDA_TRY(p, cudaMalloc(&p->own_ws, p->ws_needed));
+    p->ws = p->own_ws; p->ws_bytes = p->ws_needed;
+    return NMF_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int max_targets) {
+    if (!out) return NMF_ERR_INVALID_ARG;
+    *out = nullptr;
+    if (N < 1 || P < 1 || K < 1 || batch < 1 || max_targets < 0) return NMF_ERR_INVALID_ARG;
+    if (P % 4 != 0) return NMF_ERR_ALIGNMENT;
+    if (N > NMF_MAX_N || K > NMF_MAX_K || max_targets > 4096) return NMF_ERR_UNSUPPORTED;
+    int dev = 0;
+    if (cudaGetDevice(&dev) != cudaSuccess) return NMF_ERR_CUDA;
+    cudaDeviceProp prop;
+    if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return NMF_ERR_CUDA;
+    if (prop.major != 10) return NMF_ERR_ARCH;
+    nmf_plan* p = new (std::nothrow) nmf_plan();
+    if (!p) return NMF_ERR_INVALID_ARG;
+    p->N = N; p->P = P; p->K = K; p->batch = batch; p->max_targets = max_targets;
+    p->device = dev; p->num_sms = prop.multiProcessorCount;
+    nmf_generic_configure(p);
+    nmf_fused_configure(p);
+    p->ws_needed = plan_workspace(p);
+    *out = p;
+    return NMF_OK;
+}
+
+size_t nmf_plan_workspace_bytes(const nmf_plan* p) { return p ? p->ws_needed : 0; }
+
+int nmf_plan_set_workspace(nmf_plan* p, void* ws, size_t bytes) {
+    if (!p || !ws) return NMF_ERR_INVALID_ARG;
+    if (misaligned(ws)) return NMF_ERR_ALIGNMENT;
+    if (bytes < p->ws_needed) return NMF_ERR_WORKSPACE;
+    p->ws = ws; p->ws_bytes = bytes;
+    return NMF_OK;
+}
+
+int nmf_plan_set_stream(nmf_plan* p, void* s) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    p->stream = static_cast<cudaStream_t>(s);
+    return NMF_OK;
+}
+
+int nmf_plan_set_variant(nmf_plan* p, int v) {
+    if (!p || v < 0 || v > 2) return NMF_ERR_INVALID_ARG;
+    p->variant_req = v;
+    return NMF_OK;
+}
+
+int nmf_plan_get_variant(const nmf_plan* p) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    return use_fused(p) ? 2 : 1;
+}
+
+int nmf_plan_destroy(nmf_plan* p) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->stage) cudaFree(p->stage);
+    if (p->own_ws) cudaFree(p->own_ws);
+    delete p;
+    return NMF_OK;
+}
+
+int nmf_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters) {
+    return fit_common(p, X, Om, W, H, iters, 1);
+}
+
+int nmf_fit_batched(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    return fit_common(p, X, Om, W, H, iters, p->batch);
+}
+
+int nmf_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C, int M, int iters) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!H || !T || !C || M < 1 || M > p->max_targets || iters < 0) return NMF_ERR_INVALID_ARG;
+    if (misaligned(H) || misaligned(T) || misaligned(C) || (om && misaligned(om))) return NMF_ERR_ALIGNMENT;
+    int rc = check_ws(p);
+    if (rc) return rc;
+    if (iters == 0) return NMF_OK;
+    return nmf_generic_project(p, H, T, om, C, M, iters);
+}
+
+int nmf_subtract(nmf_plan* p, const float* H, const float* T, const float* C, const float* om,
+                 const float* factor, float fill, float* out, int M) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!H || !T || !C || !out || M < 1 || M > p->max_targets) return NMF_ERR_INVALID_ARG;
+    if (out == T || out == H) return NMF_ERR_INVALID_ARG;
+    if (misaligned(H) || misaligned(T) || misaligned(C) || misaligned(out) || (om && misaligned(om)))
+        return NMF_ERR_ALIGNMENT;
+    return nmf_aux_subtract(p, H, T, C, om, factor, fill, out, M);
+}
+
+int nmf_objective(nmf_plan* p, const float* X, const float* Om, const float* W, const float* H,
+                  double* out_host) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!X || !Om || !W || !H || !out_host) return NMF_ERR_INVALID_ARG;
+    if (misaligned(X) || misaligned(Om) || misaligned(W) || misaligned(H)) return NMF_ERR_ALIGNMENT;
+    int rc = check_ws(p);
+    if (rc) return rc;
+    return nmf_aux_objective(p, X, Om, W, H, out_host);
+}
+
+int nmf_fit_host(nmf_plan* p, const float* Xh, const float* Oh, float* Wh, float* Hh, int iters) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!Xh || !Oh || !Wh || !Hh || iters < 0) return NMF_ERR_INVALID_ARG;
+    const size_t np = nmf_align_up(sizeof(float) * (size_t)p->N * p->P, 256);
+    const size_t nk = nmf_align_up(sizeof(float) * (size_t)p->N * p->K, 256);
+    const size_t kp = nmf_align_up(sizeof(float) * (size_t)p->K * p->P, 256);
+    int rc = ensure_stage(p, 2 * np + nk + kp);
+    if (rc) return rc;
+    rc = ensure_own_ws(p);
+    if (rc) return rc;
+    char* base = static_cast<char*>(p->stage);
+    float* X = reinterpret_cast<float*>(base);
+    float* Om = reinterpret_cast<float*>(base + np);
+    float* W = reinterpret_cast<float*>(base + 2 * np);
+    float* H = reinterpret_cast<float*>(base + 2 * np + nk);
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(X, Xh, sizeof(float) * (size_t)p->N * p->P, cudaMemcpyHostToDevice, p->stream));
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(Om, Oh, sizeof(float) * (size_t)p->N * p->P, cudaMemcpyHostToDevice, p->stream));
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(W, Wh, sizeof(float) * (size_t)p->N * p->K, cudaMemcpyHostToDevice, p->stream));
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(H, Hh, sizeof(float) * (size_t)p->K * p->P, cudaMemcpyHostToDevice, p->stream));
+    rc = fit_common(p, X, Om, W, H, iters, 1);
+    if (rc) return rc;
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(Wh, W, sizeof(float) * (size_t)p->N * p->K, cudaMemcpyDeviceToHost, p->stream));
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(Hh, H, sizeof(float) * (size_t)p->K * p->P, cudaMemcpyDeviceToHost, p->stream));
+    NMF_CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    return NMF_OK;
+}
+
+int nmf_project_subtract_host(nmf_plan* p, const float* H, const float* Th, const float* oh,
+                              float* Ch, float fill, float* outh, int M, int iters) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!H || !Th || !Ch || !outh || M < 1 || M > p->max_targets || iters < 0) return NMF_ERR_INVALID_ARG;
+    const size_t mp = nmf_align_up(sizeof(float) * (size_t)M * p->P, 256);
+    const size_t mk = nmf_align_up(sizeof(float) * (size_t)M * p->K, 256);
+    int rc = ensure_stage(p, 3 * mp + mk);
+    if (rc) return rc;
+    rc = ensure_own_ws(p);
+    if (rc) return rc;
+    char* base = static_cast<char*>(p->stage);
+    float* T = reinterpret_cast<float*>(base);
+    float* om = oh ? reinterpret_cast<float*>(base + mp) : nullptr;
+    float* out = reinterpret_cast<float*>(base + 2 * mp);
+    float* C = reinterpret_cast<float*>(base + 3 * mp);
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(T, Th, sizeof(float) * (size_t)M * p->P, cudaMemcpyHostToDevice, p->stream));
+    if (oh) NMF_CUDA_TRY(p, cudaMemcpyAsync(om, oh, sizeof(float) * (size_t)M * p->P, cudaMemcpyHostToDevice, p->stream));
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(C, Ch, sizeof(float) * (size_t)M * p->K, cudaMemcpyHostToDevice, p->stream));
+    rc = nmf_project(p, H, T, om, C, M, iters);
+    if (rc) return rc;
+    rc = nmf_subtract(p, H, T, C, om, nullptr, fill, out, M);
+    if (rc) return rc;
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(Ch, C, sizeof(float) * (size_t)M * p->K, cudaMemcpyDeviceToHost, p->stream));
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(outh, out, sizeof(float) * (size_t)M * p->P, cudaMemcpyDeviceToHost, p->stream));
+    NMF_CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    return NMF_OK;
+}
+
+long long nmf_plan_launch_count(const nmf_plan* p) { return p ? p->launches : 0; }
+
+const char* nmf_status_string(int code) {
+    switch (code) {
+        case NMF_OK: return "NMF_OK";
+        case NMF_ERR_INVALID_ARG: return "NMF_ERR_INVALID_ARG: null pointer or size out of range";
+        case NMF_ERR_ALIGNMENT: return "NMF_ERR_ALIGNMENT: pointer not 16-byte aligned or P % 4 != 0";
+        case NMF_ERR_UNSUPPORTED: return "NMF_ERR_UNSUPPORTED: shape beyond the compiled limits";
+        case NMF_ERR_WORKSPACE: return "NMF_ERR_WORKSPACE: workspace missing or too small";
+        case NMF_ERR_ARCH: return "NMF_ERR_ARCH: device is not compute capability 10.x (B200)";
+        case NMF_ERR_CUDA: return "NMF_ERR_CUDA: CUDA runtime or launch error";
+        default: return "unknown nmf status";
+    }
+}
+
+const char* nmf_plan_last_cuda_error(const nmf_plan* p) { return p ? p->cuda_msg.c_str() : ""; }
+
+}  // extern "C"

@@ -1,0 +1,121 @@
+// nmf_aux.cu -- PSF subtraction and the diagnostic
+// objective of Eq. 2.
+#include "nmf_common.cuh"
+
+namespace {
+
+constexpr int SUB_MC = 32;      // science frames per pass (accumulators per thread)
+constexpr int SUB_THREADS = 256;
+constexpr int OBJ_THREADS = 128;
+
+// out[m,p] = t[m,p] - f[m] * sum_k c[m,k] H[k,p]; `fill` where omega[m,p] == 0.
+// One pixel per thread, up to SUB_MC frames at once so H is streamed once per pass.
+__global__ void __launch_bounds__(SUB_THREADS)
+k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float* __restrict__ C,
+           const float* __restrict__ om, const float* __restrict__ factor, float fill,
+           float* __restrict__ out, int M, long long P, int K, int m0) {
+    extern __shared__ float cs[];   // [SUB_MC][K]
+    const int mc = min(SUB_MC, M - m0);
+    for (int i = threadIdx.x; i < SUB_MC * K; i += SUB_THREADS) {
+        int m = i / K, k = i - m * K;
+        cs[i] = m < mc ? C[(size_t)(m0 + m) * K + k] : 0.f;
+    }
+    __syncthreads();
+    const long long p = (long long)blockIdx.x * SUB_THREADS + threadIdx.x;
+    if (p >= P) return;
+    float acc[SUB_MC];
+#pragma unroll
+    for (int m = 0; m < SUB_MC; ++m) acc[m] = 0.f;
+    for (int k = 0; k < K; ++k) {
+        const float h = __ldg(H + (size_t)k * P + p);
+#pragma unroll
+        for (int m = 0; m < SUB_MC; ++m) acc[m] = fmaf(cs[m * K + k], h, acc[m]);
+    }
+#pragma unroll
+    for (int m = 0; m < SUB_MC; ++m) {
+        if (m < mc) {
+            const size_t i = (size_t)(m0 + m) * P + p;
+            const bool live = om ? (om[i] > 0.f) : true;
+            const float f = factor ? factor[m0 + m] : 1.f;
+            out[i] = live ? (T[i] - f * acc[m]) : fill;
+        }
+    }
+}
+
+// sum_{Om>0} Om (X - W H)^2 in fp64; one pixel per thread, per-block partial.
+__global__ void __launch_bounds__(OBJ_THREADS)
+k_objective(const float* __restrict__ X, const float* __restrict__ Om, const float* __restrict__ W,
+            const float* __restrict__ H, double* __restrict__ partial, int N, long long P, int K) {
+    extern __shared__ __align__(16) float smem[];
+    float* ws = smem;                       // [N][K]
+    float* hs = smem + (size_t)N * K;       // [K][OBJ_THREADS]
+    __shared__ double red[OBJ_THREADS / 32];
+    for (int i = threadIdx.x; i < N * K; i += OBJ_THREADS) ws[i] = W[i];
+    const long long p = (long long)blockIdx.x * OBJ_THREADS + threadIdx.x;
+    const bool active = p < P;
+    for (int k = 0; k < K; ++k) hs[k * OBJ_THREADS + threadIdx.x] = active ? H[(size_t)k * P + p] : 0.f;
+    __syncthreads();
+    double f = 0.0;
+    if (active) {
+        for (int n = 0; n < N; ++n) {
+            const float o = Om[(size_t)n * P + p];
+            if (!(o > 0.f)) continue;
+            double s = 0.0;
+            for (int k = 0; k < K; ++k) s += (double)ws[n * K + k] * (double)hs[k * OBJ_THREADS + threadIdx.x];
+            const double d = (double)X[(size_t)n * P + p] - s;
+            f += (double)o * d * d;
+        }
+    }
+    for (int d = 16; d > 0; d >>= 1) f += __shfl_xor_sync(0xffffffffu, f, d);
+    if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = f;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int w = 0; w < OBJ_THREADS / 32; ++w) t += red[w];
+        partial[blockIdx.x] = t;
+    }
+}
+
+}  // namespace
+
+size_t nmf_aux_workspace(const nmf_plan* p) {
+    return sizeof(double) * (size_t)((p->P + OBJ_THREADS - 1) / OBJ_THREADS);
+}
+
+int nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C, const float* om,
+                     const float* factor, float fill, float* out, int M) {
+    const unsigned grid = (unsigned)((p->P + SUB_THREADS - 1) / SUB_THREADS);
+    const size_t smem = sizeof(float) * SUB_MC * p->K;
+    for (int m0 = 0; m0 < M; m0 += SUB_MC) {
+        k_subtract<<<grid, SUB_THREADS, smem, p->stream>>>(H, T, C, om, factor, fill, out, M, p->P, p->K, m0);
+        p->launches++;
+    }
+    NMF_CUDA_TRY(p, cudaGetLastError());
+    return NMF_OK;
+}
+
+int nmf_aux_objective(nmf_plan* p, const float* X, const float* Om, const float* W, const float* H,
+                      double* out_host) {
+    const unsigned grid = (unsigned)((p->P + OBJ_THREADS - 1) / OBJ_THREADS);
+    const size_t smem = sizeof(float) * ((size_t)p->N * p->K + (size_t)p->K * OBJ_THREADS);
+    static bool attr_done = false;
+    if (!attr_done) {
+        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_objective, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
+        attr_done = true;
+    }
+    // objective partials live at the tail of the workspace
+    double* partial = reinterpret_cast<double*>(static_cast<char*>(p->ws) + (p->ws_needed - nmf_aux_workspace(p)));
+    k_objective<<<grid, OBJ_THREADS, smem, p->stream>>>(X, Om, W, H, partial, p->N, p->P, p->K);
+    p->launches++;
+    NMF_CUDA_TRY(p, cudaGetLastError());
+    double* host = nullptr;
+    NMF_CUDA_TRY(p, cudaMallocHost(&host, sizeof(double) * grid));
+    cudaError_t e = cudaMemcpyAsync(host, partial, sizeof(double) * grid, cudaMemcpyDeviceToHost, p->stream);
+    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
+    if (e != cudaSuccess) { cudaFreeHost(host); return nmf_cuda_fail(p, e); }
+    double f = 0.0;
+    for (unsigned i = 0; i < grid; ++i) f += host[i];   // fixed order
+    cudaFreeHost(host);
+    *out_host = f;
+    return NMF_OK;
+}

@@ -1,0 +1,73 @@
+// nmf_common.cuh -- shared host/device declarations of the sm_100a NMF library.
+// (Library-internal; the public boundary is include/nmf.h.)
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+#include <stddef.h>
+#include <string>
+#include "../../include/nmf.h"
+
+#define NMF_EPS 1e-30f   // ratio guard: num / max(den, NMF_EPS)   (reading G4)
+
+// ---------------------------------------------------------------------------
+// plan
+// ---------------------------------------------------------------------------
+struct nmf_plan {
+    int N = 0, K = 0, batch = 1, max_targets = 0;
+    long long P = 0;
+    int device = 0;
+    int num_sms = 148;
+    cudaStream_t stream = nullptr;
+    void* ws = nullptr;
+    size_t ws_bytes = 0;
+    size_t ws_needed = 0;
+    int variant_req = 0;          // 0 auto, 1 generic, 2 fused
+    long long launches = 0;
+    int sticky = 0;               // first CUDA error seen (nmf_status)
+    std::string cuda_msg;
+
+    // generic-path geometry (see nmf_generic.cu)
+    int g_kc = 0, g_ks = 0;       // per-thread K chunk, lanes per item
+    int g_parts_fit = 0;          // pixel-range partitions of the W half-step (fit)
+    int g_parts_proj = 0;         // same for projection
+    // fused-path geometry (see nmf_fused.cu)
+    int f_kp = 0;                 // padded K of the fused instantiation (0 = unavailable)
+    int f_ctas = 0;               // persistent CTAs per problem
+    // host staging for the *_host entry points (plan-owned device buffers)
+    void* stage = nullptr;
+    size_t stage_bytes = 0;
+    void* own_ws = nullptr;       // workspace allocated by a *_host call when none was set
+};
+
+static inline int nmf_cuda_fail(nmf_plan* p, cudaError_t e) {
+    if (p && !p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = cudaGetErrorString(e); }
+    return NMF_ERR_CUDA;
+}
+#define NMF_CUDA_TRY(plan, expr)                                   \
+    do { cudaError_t _e = (expr);                                  \
+         if (_e != cudaSuccess) return nmf_cuda_fail((plan), _e); } while (0)
+
+static inline size_t nmf_align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ---------------------------------------------------------------------------
+// launchers implemented in the .cu files (all enqueue on plan->stream)
+// ---------------------------------------------------------------------------
+// generic two-kernel path
+void   nmf_generic_configure(nmf_plan* p);
+size_t nmf_generic_workspace(const nmf_plan* p);
+int    nmf_generic_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
+                       int iters, int batch);
+int    nmf_generic_project(nmf_plan* p, const float* H, const float* T, const float* om,
+                           float* C, int M, int iters);
+// fused per-pixel-tile path
+void   nmf_fused_configure(nmf_plan* p);
+size_t nmf_fused_workspace(const nmf_plan* p);
+bool   nmf_fused_available(const nmf_plan* p);
+int    nmf_fused_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
+                     int iters, int batch);
+// auxiliaries
+size_t nmf_aux_workspace(const nmf_plan* p);
+int    nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C,
+                        const float* om, const float* factor, float fill, float* out, int M);
+int    nmf_aux_objective(nmf_plan* p, const float* X, const float* Om, const float* W,
+                         const float* H, double* out_host);

@@ -1,0 +1,184 @@
+"""Thin ctypes binding of include/nmf.h -- argument marshalling only.
+
+Every step of the hot path runs in the CUDA kernels of libnmf_b200.so; this
+module passes torch device pointers, sizes and the current CUDA stream across
+the C-ABI and owns nothing but the plan handle and its workspace tensor.  There
+is no CPU fallback: a missing library or a non-CUDA tensor raises.
+
+Names mirror the C entry points: Plan(N,P,K) ~ nmf_plan_create, Plan.fit ~ nmf_fit,
+Plan.fit_batched, Plan.project ~ nmf_project, Plan.subtract ~ nmf_subtract,
+Plan.objective ~ nmf_objective, Plan.fit_host / Plan.project_subtract_host.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from typing import Optional
+
+import torch
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "libnmf_b200.so")
+
+SYMBOLS = (
+    "nmf_plan_create", "nmf_plan_workspace_bytes", "nmf_plan_set_workspace", "nmf_plan_set_stream",
+    "nmf_plan_set_variant", "nmf_plan_get_variant", "nmf_plan_destroy", "nmf_fit", "nmf_fit_batched",
+    "nmf_project", "nmf_subtract", "nmf_objective", "nmf_fit_host", "nmf_project_subtract_host",
+    "nmf_plan_launch_count", "nmf_status_string", "nmf_plan_last_cuda_error",
+)
+
+_lib = None
+_vp, _ci, _cll, _cf = ctypes.c_void_p, ctypes.c_int, ctypes.c_longlong, ctypes.c_float
+
+
+class NMFError(RuntimeError):
+    def __init__(self, code: int, detail: str = ""):
+        self.code = code
+        msg = lib().nmf_status_string(code).decode()
+        super().__init__(f"{msg}{(' -- ' + detail) if detail else ''}")
+
+
+def lib():
+    """Load libnmf_b200.so (fails loudly when the CUDA extension is missing)."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise ImportError(f"{LIB_PATH} not built: run `python -m paper_2309_04623_b200.build` "
+                              "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        L.nmf_plan_create.argtypes = [ctypes.POINTER(_vp), _ci, _cll, _ci, _ci, _ci]
+        L.nmf_plan_workspace_bytes.argtypes = [_vp]; L.nmf_plan_workspace_bytes.restype = ctypes.c_size_t
+        L.nmf_plan_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
+        L.nmf_plan_set_stream.argtypes = [_vp, _vp]
+        L.nmf_plan_set_variant.argtypes = [_vp, _ci]
+        L.nmf_plan_get_variant.argtypes = [_vp]
+        L.nmf_plan_destroy.argtypes = [_vp]
+        L.nmf_fit.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci]
+        L.nmf_fit_batched.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci]
+        L.nmf_project.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci]
+        L.nmf_subtract.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _cf, _vp, _ci]
+        L.nmf_objective.argtypes = [_vp, _vp, _vp, _vp, _vp, ctypes.POINTER(ctypes.c_double)]
+        L.nmf_fit_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci]
+        L.nmf_project_subtract_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _cf, _vp, _ci, _ci]
+        L.nmf_plan_launch_count.argtypes = [_vp]; L.nmf_plan_launch_count.restype = _cll
+        L.nmf_status_string.argtypes = [_ci]; L.nmf_status_string.restype = ctypes.c_char_p
+        L.nmf_plan_last_cuda_error.argtypes = [_vp]; L.nmf_plan_last_cuda_error.restype = ctypes.c_char_p
+        _lib = L
+    return _lib
+
+
+def _dev(t: torch.Tensor, shape=None) -> int:
+    if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float32 CUDA tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+def _host(t: torch.Tensor, shape=None) -> int:
+    if not (isinstance(t, torch.Tensor) and not t.is_cuda and t.dtype == torch.float32 and t.is_contiguous()):
+        raise TypeError("expected a contiguous float32 host tensor")
+    if shape is not None and tuple(t.shape) != tuple(shape):
+        raise ValueError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
+    return t.data_ptr()
+
+
+class Plan:
+    """nmf_plan for problems of shape (N frames, P pixels, K components)."""
+
+    def __init__(self, N: int, P: int, K: int, batch: int = 1, max_targets: int = 0,
+                 device: Optional[torch.device] = None, variant: int = 0):
+        self._h = _vp()
+        self.N, self.P, self.K, self.batch, self.max_targets = N, P, K, batch, max_targets
+        self.device = torch.device("cuda", torch.cuda.current_device()) if device is None else torch.device(device)
+        with torch.cuda.device(self.device):
+            rc = lib().nmf_plan_create(ctypes.byref(self._h), N, P, K, batch, max_targets)
+        if rc:
+            self._h = _vp()
+            raise NMFError(rc)
+        nbytes = lib().nmf_plan_workspace_bytes(self._h)
+        self.workspace = torch.empty(max(nbytes, 16), dtype=torch.uint8, device=self.device)
+        self._check(lib().nmf_plan_set_workspace(self._h, self.workspace.data_ptr(), self.workspace.numel()))
+        if variant:
+            self._check(lib().nmf_plan_set_variant(self._h, variant))
+
+    # -- plumbing ---------------------------------------------------------
+    def _check(self, rc: int):
+        if rc:
+            raise NMFError(rc, lib().nmf_plan_last_cuda_error(self._h).decode() if self._h else "")
+
+    def _sync_stream(self):
+        self._check(lib().nmf_plan_set_stream(self._h, torch.cuda.current_stream(self.device).cuda_stream))
+
+    @property
+    def variant(self) -> int:
+        return lib().nmf_plan_get_variant(self._h)
+
+    @property
+    def launch_count(self) -> int:
+        return int(lib().nmf_plan_launch_count(self._h))
+
+    def close(self):
+        if getattr(self, "_h", None) and self._h.value:
+            lib().nmf_plan_destroy(self._h)
+            self._h = _vp()
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    # -- the calls of include/nmf.h ------------------------------------------
+    def fit(self, X, Omega, W, H, iters: int):
+        self._sync_stream()
+        self._check(lib().nmf_fit(self._h, _dev(X, (self.N, self.P)), _dev(Omega, (self.N, self.P)),
+                                  _dev(W, (self.N, self.K)), _dev(H, (self.K, self.P)), iters))
+
+    def fit_batched(self, X, Omega, W, H, iters: int):
+        B = self.batch
+        self._sync_stream()
+        self._check(lib().nmf_fit_batched(self._h, _dev(X, (B, self.N, self.P)), _dev(Omega, (B, self.N, self.P)),
+                                          _dev(W, (B, self.N, self.K)), _dev(H, (B, self.K, self.P)), iters))
+
+    def project(self, H, target, omega, coef, iters: int):
+        M = target.shape[0]
+        self._sync_stream()
+        self._check(lib().nmf_project(self._h, _dev(H, (self.K, self.P)), _dev(target, (M, self.P)),
+                                      None if omega is None else _dev(omega, (M, self.P)),
+                                      _dev(coef, (M, self.K)), M, iters))
+
+    def subtract(self, H, target, coef, omega=None, factor=None, fill: float = 0.0, out=None):
+        M = target.shape[0]
+        if out is None:
+            out = torch.empty_like(target)
+        self._sync_stream()
+        self._check(lib().nmf_subtract(self._h, _dev(H, (self.K, self.P)), _dev(target, (M, self.P)),
+                                       _dev(coef, (M, self.K)),
+                                       None if omega is None else _dev(omega, (M, self.P)),
+                                       None if factor is None else _dev(factor, (M,)),
+                                       float(fill), _dev(out, (M, self.P)), M))
+        return out
+
+    def objective(self, X, Omega, W, H) -> float:
+        out = ctypes.c_double(0.0)
+        self._sync_stream()
+        self._check(lib().nmf_objective(self._h, _dev(X, (self.N, self.P)), _dev(Omega, (self.N, self.P)),
+                                        _dev(W, (self.N, self.K)), _dev(H, (self.K, self.P)), ctypes.byref(out)))
+        return out.value
+
+    def fit_host(self, X, Omega, W, H, iters: int):
+        """Host-buffer end-to-end fit (H2D + fit + D2H inside the call; synchronises)."""
+        self._sync_stream()
+        with torch.cuda.device(self.device):
+            self._check(lib().nmf_fit_host(self._h, _host(X, (self.N, self.P)), _host(Omega, (self.N, self.P)),
+                                           _host(W, (self.N, self.K)), _host(H, (self.K, self.P)), iters))
+
+    def project_subtract_host(self, H_dev, target, omega, coef, out, iters: int, fill: float = 0.0):
+        M = target.shape[0]
+        self._sync_stream()
+        with torch.cuda.device(self.device):
+            self._check(lib().nmf_project_subtract_host(
+                self._h, _dev(H_dev, (self.K, self.P)), _host(target, (M, self.P)),
+                None if omega is None else _host(omega, (M, self.P)), _host(coef, (M, self.K)),
+                float(fill), _host(out, (M, self.P)), M, iters))

@@ -1,0 +1,133 @@
+"""T2: properties of the CUDA path that hold at any size (no oracle run needed) and the
+degenerate / ragged / error cases of the boundary."""
+import ctypes
+
+import numpy as np
+import pytest
+import torch
+
+from oracle import nmf_oracle as orc
+from paper_2309_04623_b200 import inputs, nmf
+from gpu_util import TOL_FACTOR, check_fit_parity, dev, gpu_fit, rel
+
+pytestmark = pytest.mark.gpu
+VARIANTS = [1, 0]
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_bitwise_determinism_and_resume(variant):
+    p = inputs.make_miri(N=40, S=96, K=12, M=1)
+    W1, H1, plan = gpu_fit(p, 40, variant)
+    W2, H2, _ = gpu_fit(p, 40, variant, plan)
+    assert np.array_equal(W1, W2) and np.array_equal(H1, H2)
+    # checkpoint/resume: 20 + 20 iterations == 40 iterations, bitwise
+    X, Om, W, H = dev(p.X), dev(p.Omega), dev(p.W0), dev(p.H0)
+    plan.fit(X, Om, W, H, 20); plan.fit(X, Om, W, H, 20)
+    torch.cuda.synchronize()
+    assert np.array_equal(W.cpu().numpy(), W1) and np.array_equal(H.cpu().numpy(), H1)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("garbage", [np.nan, 1e30, np.inf])
+def test_mask_invariance_bitwise(variant, garbage):
+    """Entries with Omega == 0 must not influence anything, even NaN/Inf."""
+    p = inputs.make_miri(N=32, S=64, K=10, M=2)
+    W1, H1, plan = gpu_fit(p, 25, variant)
+    q = inputs.make_miri(N=32, S=64, K=10, M=2)
+    q.X[q.Omega == 0] = garbage
+    W2, H2, _ = gpu_fit(q, 25, variant, plan)
+    assert np.array_equal(W1, W2) and np.array_equal(H1, H2)
+    q.T[q.omega_t == 0] = garbage
+    Hd = dev(H1)
+    C1, C2 = dev(p.C0), dev(p.C0)
+    plan.project(Hd, dev(p.T), dev(p.omega_t), C1, 20)
+    plan.project(Hd, dev(q.T), dev(q.omega_t), C2, 20)
+    assert torch.equal(C1, C2)
+    out = plan.subtract(Hd, dev(q.T), C2, dev(q.omega_t), None, -1.0)
+    assert torch.isfinite(out).all() and bool((out[dev(q.omega_t) == 0] == -1.0).all())
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+def test_power_of_two_homogeneity_bitwise(variant):
+    p = inputs.make_tiny()
+    W1, H1, plan = gpu_fit(p, 30, variant)
+    q = inputs.make_tiny(); q.X *= np.float32(4); q.W0 *= np.float32(4)
+    W2, H2, _ = gpu_fit(q, 30, variant, plan)
+    assert np.array_equal(H1, H2) and np.array_equal(W2, W1 * np.float32(4))
+    q = inputs.make_tiny(); q.Omega *= np.float32(0.125)
+    W3, H3, _ = gpu_fit(q, 30, variant, plan)
+    assert np.array_equal(H1, H3) and np.array_equal(W1, W3)
+
+
+@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("N,P,K", [(1, 4, 1), (3, 36, 2), (7, 132, 5), (33, 1028, 9), (65, 4100, 17),
+                                   (129, 2052, 33), (200, 996, 50), (256, 516, 128), (225, 260, 53)])
+def test_ragged_and_extreme_shapes(variant, N, P, K):
+    """N, K, P off every tile size; K=1; the compiled maxima N=256, K=128; row-varying zeros in Omega."""
+    rng = np.random.default_rng(N * 1000 + K)
+    X = (rng.random((N, P)) * 10).astype(np.float32)
+    Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.25)).astype(np.float32)
+    Om[:, P // 2] = 0            # one fully masked column
+    W0 = (0.1 + 0.9 * rng.random((N, K))).astype(np.float32)
+    H0 = (0.1 + 0.9 * rng.random((K, P))).astype(np.float32)
+    plan = nmf.Plan(N, P, K, variant=variant)
+    Xd, Od, Wd, Hd = dev(X), dev(Om), dev(W0), dev(H0)
+    plan.fit(Xd, Od, Wd, Hd, 8)
+    torch.cuda.synchronize()
+    Wo, Ho = orc.fit(X, Om, W0, H0, 8)
+    Hg = Hd.cpu().numpy()
+    assert rel(Wd.cpu().numpy(), Wo) <= TOL_FACTOR and rel(Hg, Ho) <= TOL_FACTOR
+    assert np.all(Hg[:, P // 2] == 0.0)     # G4: fully masked column -> exactly 0
+
+
+def test_zero_entries_stay_zero_and_empty_iters():
+    p = inputs.make_tiny()
+    p.W0[2, 1] = 0.0; p.H0[3, 77] = 0.0
+    W, H, plan = gpu_fit(p, 10)
+    assert W[2, 1] == 0.0 and H[3, 77] == 0.0
+    W0, H0, _ = gpu_fit(p, 0, plan=plan)
+    assert np.array_equal(W0, p.W0) and np.array_equal(H0, p.H0)
+
+
+def test_objective_monotone_on_gpu_iterates():
+    """fp32 iterates still decrease the fp64-evaluated objective every iteration (P1 on the device path)."""
+    p = inputs.make_tiny()
+    plan = nmf.Plan(p.N, p.P, p.K)
+    X, Om, W, H = dev(p.X), dev(p.Omega), dev(p.W0), dev(p.H0)
+    prev = plan.objective(X, Om, W, H)
+    for _ in range(25):
+        plan.fit(X, Om, W, H, 1)
+        f = plan.objective(X, Om, W, H)
+        assert f <= prev * (1 + 1e-6)
+        prev = f
+
+
+def test_error_codes():
+    L = nmf.lib()
+    p = inputs.make_tiny()
+    plan = nmf.Plan(p.N, p.P, p.K, max_targets=2)
+    X, Om, W, H = dev(p.X), dev(p.Omega), dev(p.W0), dev(p.H0)
+    h = plan._h
+    assert L.nmf_fit(h, None, Om.data_ptr(), W.data_ptr(), H.data_ptr(), 1) == -1
+    assert L.nmf_fit(h, X.data_ptr(), Om.data_ptr(), W.data_ptr(), H.data_ptr(), -1) == -1
+    assert L.nmf_fit(h, X.data_ptr() + 4, Om.data_ptr(), W.data_ptr(), H.data_ptr(), 1) == -2
+    assert L.nmf_project(h, H.data_ptr(), X.data_ptr(), None, W.data_ptr(), 3, 1) == -1    # M > max_targets
+    assert L.nmf_plan_set_workspace(h, plan.workspace.data_ptr(), 8) == -4
+    h2 = ctypes.c_void_p()
+    assert L.nmf_plan_create(ctypes.byref(h2), p.N, p.P, p.K, 1, 0) == 0
+    assert L.nmf_fit(h2, X.data_ptr(), Om.data_ptr(), W.data_ptr(), H.data_ptr(), 1) == -4  # no workspace
+    assert L.nmf_plan_destroy(h2) == 0
+    with pytest.raises(TypeError):
+        plan.fit(X.cpu(), Om, W, H, 1)
+
+
+def test_host_entry_points_match_device_path():
+    p = inputs.make_miri(N=24, S=64, K=8, M=3)
+    Wd, Hd, plan = gpu_fit(p, 15)
+    Wh, Hh = torch.from_numpy(p.W0.copy()), torch.from_numpy(p.H0.copy())
+    plan.fit_host(torch.from_numpy(p.X), torch.from_numpy(p.Omega), Wh, Hh, 15)
+    assert np.array_equal(Wh.numpy(), Wd) and np.array_equal(Hh.numpy(), Hd)
+    C = torch.from_numpy(p.C0.copy()); out = torch.empty(p.M, p.P)
+    plan.project_subtract_host(dev(Hd), torch.from_numpy(p.T), torch.from_numpy(p.omega_t), C, out, 30)
+    Co = orc.project(Hd, p.T, p.omega_t, p.C0, 30)
+    assert rel(C.numpy(), Co) <= TOL_FACTOR
