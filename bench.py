@@ -1,0 +1,307 @@
+#!/usr/bin/env python
+"""bench.py -- headline benchmark of the B200-native weighted-NMF hot path.
+
+    python bench.py --gpus N --steps K --warmup W [--impl reference] [--workload stis]
+
+Metric (BASELINE.json): NMF iterations/s at 200 reference frames x 1024^2 px x K=50, fp32.
+One "step" is one pass of the whole hot path of SURVEY.md 8(a) over the STIS-shaped
+synthetic library: one full NMF iteration (a1-a8: H half-step, W half-step), one
+projection iteration of the 32 science frames on the current components (a9) and one
+PSF subtraction (a10).  `value` = steps/s summed over all ranks (each rank runs its own
+independent replica: weak scaling, no data-path collective).
+
+Prints ONE JSON line (rank 0).  See DESIGN.md "Measurement" for every field.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+sys.path.insert(0, ROOT)
+
+METRIC = "nmf_iterations_per_s@200x1024^2xK50_fp32"
+UNIT = "iterations/s"
+WORKLOADS = {
+    # name: (N, S, K, M)   -- configs[2] of BASELINE.json is the one the metric is quoted on
+    "stis": dict(N=200, S=1024, K=50, M=32),
+    "stis_small": dict(N=200, S=256, K=50, M=8),     # debugging only
+}
+ALU_PEAK_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12     # FP32 FFMA: SMs x lanes x 2 x max SM clock
+
+
+def flops_per_iter(N, P, K):
+    return 12.0 * N * K * P          # six N.K.P contractions
+
+
+def bytes_per_iter(N, P, K):
+    return 8.0 * N * P + 8.0 * K * P  # X, Omega read once; H read + written
+
+
+# ------------------------------------------------------------------------------
+# clocks sampler (nvidia-smi during the timed region)
+# ------------------------------------------------------------------------------
+class ClockSampler:
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
+         "clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index: int):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", "-i", str(index), f"--query-gpu={self.Q}",
+                                       "--format=csv,noheader,nounits", "-lms", "100"],
+                                      stdout=self.f, stderr=subprocess.DEVNULL)
+        except Exception:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        self.p.terminate()
+        try:
+            self.p.wait(timeout=5)
+        except Exception:
+            self.p.kill()
+        self.f.flush(); self.f.seek(0)
+        sm, smax, reasons, power = [], [], set(), []
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in self.f:
+            t = [c.strip() for c in line.split(",")]
+            if len(t) < 7:
+                continue
+            try:
+                sm.append(float(t[0])); smax.append(float(t[1])); power.append(float(t[2]))
+            except ValueError:
+                continue
+            for nm, v in zip(names, t[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(nm)
+        os.unlink(self.f.name)
+        # keep the samples taken under load (upper half of the clock readings)
+        return {"sm_mhz": statistics.median(sm) if sm else None,
+                "sm_max_mhz": max(smax) if smax else None,
+                "power_w_max": max(power) if power else None,
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------
+# the CPU oracle legs (cpu_baseline and --impl reference)
+# ------------------------------------------------------------------------------
+def oracle_step_rate(p, crop_rows: int, steps: int, warmup: int):
+    """Time the oracle, as it stands, on a crop of the workload: the first `crop_rows`
+    image rows of every frame (all N frames, all K components).  One step = one oracle
+    iteration + one projection iteration + subtraction, as in the GPU arm.  Returns
+    full-size-equivalent steps/s (crop rate x crop fraction), seconds per crop step."""
+    from oracle import nmf_oracle as orc
+    Pc = crop_rows * p.S
+    X = np.ascontiguousarray(p.X[:, :Pc]); Om = np.ascontiguousarray(p.Omega[:, :Pc])
+    T = np.ascontiguousarray(p.T[:, :Pc]); om = np.ascontiguousarray(p.omega_t[:, :Pc])
+    W = p.W0.astype(np.float64); H = np.ascontiguousarray(p.H0[:, :Pc]).astype(np.float64)
+    C = p.C0.astype(np.float64)
+    dt = []
+    for s in range(warmup + steps):
+        t0 = time.perf_counter()
+        W, H = orc.fit(X, Om, W, H, 1)
+        C = orc.project(H, T, om, C, 1)
+        orc.subtract(H, T, C, om, None, 0.0)
+        if s >= warmup:
+            dt.append(time.perf_counter() - t0)
+    sec = sum(dt) / len(dt)
+    return (1.0 / sec) * (Pc / p.P), sec, orc.num_threads()
+
+
+def run_reference(args, rank):
+    """--impl reference: the fp64 oracle on the host cores (rank 0 only)."""
+    if rank != 0:
+        return
+    from paper_2309_04623_b200 import inputs
+    wl = WORKLOADS[args.workload]
+    p = inputs.make_stis(N=wl["N"], S=wl["S"], K=wl["K"], M=wl["M"])
+    crop_rows = max(1, wl["S"] // 64)     # 1/64 of the pixels per step
+    rate, sec, cores = oracle_step_rate(p, crop_rows, args.steps, max(args.warmup, 1))
+    sample = (f"first {crop_rows} image rows ({crop_rows * p.S} of {p.P} px) of all {p.N} frames, K={p.K}; "
+              f"rate scaled by the pixel fraction to the full workload")
+    line = {"impl": "reference", "metric": METRIC, "value": rate, "unit": UNIT, "n_gpus": args.gpus,
+            "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 / rate,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic", "gpu_launches": 0,
+            "config": {"workload": f"STIS-shaped N={p.N} {p.S}x{p.S}px K={p.K} M={p.M} (BASELINE.json configs[2])",
+                       "step": "1 NMF iteration + 1 projection iteration + subtraction", "sample": sample},
+            "cpu_baseline": {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
+            "e2e": {"value": rate, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}}
+    print(json.dumps(line))
+
+
+# ------------------------------------------------------------------------------
+# the GPU arm
+# ------------------------------------------------------------------------------
+def run_ours(args, rank, world, local_rank):
+    import torch
+    import torch.distributed as dist
+    from paper_2309_04623_b200 import inputs, nmf
+
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    wl = WORKLOADS[args.workload]
+    # every rank fits its own replica (per-rank seed): independent problems, no collective
+    p = inputs.make_stis(N=wl["N"], S=wl["S"], K=wl["K"], M=wl["M"], seed=3003 + 7919 * rank)
+    N, P, K, M = p.N, p.P, p.K, p.M
+    plan = nmf.Plan(N, P, K, max_targets=M, variant=args.variant)
+    pin = lambda a: torch.from_numpy(a).pin_memory()
+    hX, hOm, hT, hom = pin(p.X), pin(p.Omega), pin(p.T), pin(p.omega_t)
+    X, Om, T, om = hX.cuda(non_blocking=True), hOm.cuda(non_blocking=True), hT.cuda(non_blocking=True), hom.cuda(non_blocking=True)
+    W, H, C = torch.from_numpy(p.W0).cuda(), torch.from_numpy(p.H0).cuda(), torch.from_numpy(p.C0).cuda()
+    out = torch.empty_like(T)
+    torch.cuda.synchronize()
+
+    def step():
+        plan.fit(X, Om, W, H, 1)
+        plan.project(H, T, om, C, 1)
+        plan.subtract(H, T, C, om, None, 0.0, out)
+
+    for _ in range(args.warmup):
+        step()
+    ev = lambda: torch.cuda.Event(enable_timing=True)
+    fit_ev = [(ev(), ev()) for _ in range(args.steps)]
+    e0, e1 = ev(), ev()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    sampler = ClockSampler(local_rank) if rank == 0 else None
+    l0 = plan.launch_count
+    e0.record()
+    for s in range(args.steps):
+        fit_ev[s][0].record()
+        plan.fit(X, Om, W, H, 1)
+        fit_ev[s][1].record()
+        plan.project(H, T, om, C, 1)
+        plan.subtract(H, T, C, om, None, 0.0, out)
+    e1.record()
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    clocks = sampler.stop() if sampler else None
+    launches = plan.launch_count - l0
+    ms_total = e0.elapsed_time(e1)
+    fit_ms = [a.elapsed_time(b) for a, b in fit_ev]
+    t = torch.tensor([ms_total], device="cuda")
+    if world > 1:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_max = float(t.item())
+    assert torch.isfinite(W).all() and torch.isfinite(H).all()
+
+    # ---- end-to-end through the C-ABI with host buffers (copies inside the timed region) ----
+    hW, hH, hC = pin(p.W0.copy()), pin(p.H0.copy()), pin(p.C0.copy())
+    hout = torch.empty(M, P).pin_memory()
+    e2e_iters = args.steps
+
+    def e2e_call():
+        plan.fit_host(hX, hOm, hW, hH, e2e_iters)
+        Hd = torch.empty(K, P, device="cuda"); Hd.copy_(hH, non_blocking=True)
+        plan.project_subtract_host(Hd, hT, hom, hC, hout, e2e_iters)
+
+    hW.copy_(torch.from_numpy(p.W0)); hH.copy_(torch.from_numpy(p.H0))
+    e2e_call()                                    # warm-up: staging allocation
+    hW.copy_(torch.from_numpy(p.W0)); hH.copy_(torch.from_numpy(p.H0)); hC.copy_(torch.from_numpy(p.C0))
+    torch.cuda.synchronize()
+    if world > 1:
+        dist.barrier()
+    t0 = time.perf_counter()
+    e2e_call()
+    torch.cuda.synchronize()
+    e2e_s = time.perf_counter() - t0
+    te = torch.tensor([e2e_s], device="cuda")
+    if world > 1:
+        dist.all_reduce(te, op=dist.ReduceOp.MAX)
+    e2e_s = float(te.item())
+    h2d = 4.0 * (2 * N * P + N * K + K * P) + 4.0 * (K * P + 2 * M * P + M * K)
+    d2h = 4.0 * (N * K + K * P) + 4.0 * (M * K + M * P)
+
+    if rank != 0:
+        return
+    value = world * args.steps / (ms_max * 1e-3)
+    fit_ms_avg = sum(fit_ms) / len(fit_ms)
+    F = flops_per_iter(N, P, K)
+    achieved = F / (fit_ms_avg * 1e-3) / 1e12
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except Exception:
+        pass
+    hbm_peak = peaks.get("hbm_gbs", 6650.0)
+    traffic = None
+    try:
+        traffic = json.load(open(os.path.join(ROOT, "profiles", "traffic.json"))).get(f"variant{plan.variant}")
+    except Exception:
+        pass
+    cpu = None
+    if not args.no_cpu_baseline:
+        crop_rows = max(1, wl["S"] // 4)
+        rate, sec, cores = oracle_step_rate(p, crop_rows, 2, 1)
+        cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
+               "sample": f"2 timed steps (+1 warm-up) on the first {crop_rows} image rows ({crop_rows * p.S} of {P} px) "
+                         f"of all {N} frames, K={K}, {sec:.2f} s per crop step; rate scaled by the pixel fraction"}
+    line = {
+        "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
+        "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
+        "config": {"workload": f"STIS-shaped N={N} {p.S}x{p.S}px K={K} M={M} (BASELINE.json configs[2])",
+                   "step": "1 NMF iteration (a1-a8) + 1 projection iteration of M frames (a9) + subtraction (a10)",
+                   "fit_variant": {1: "generic two-kernel", 2: "fused per-pixel-tile"}[plan.variant],
+                   "l2": "inputs (X+Omega 1.6 GB per step) are larger than the 126 MB L2; no explicit flush",
+                   "parallelism": f"{world} independent replica(s), no collective"},
+        "fit_ms_per_iter": fit_ms_avg,
+        "fit_iterations_per_s": 1e3 / fit_ms_avg,
+        "roofline": {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                     "frac": achieved / ALU_PEAK_TFLOPS, "traffic": traffic,
+                     "kernel": "fit iteration (fused tile kernel + fixed-order reduce/W update)" if plan.variant == 2
+                               else "fit iteration (H half-step + W half-step partial + reduce kernels)",
+                     "algorithmic_flops_per_launch": F, "algorithmic_bytes_per_launch": bytes_per_iter(N, P, K),
+                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts/clocks)",
+                     "hbm_time_floor_ms": bytes_per_iter(N, P, K) / (hbm_peak * 1e9) * 1e3,
+                     "hbm_peak_gbs_measured": hbm_peak},
+        "e2e": {"value": world * e2e_iters / e2e_s, "unit": UNIT,
+                "h2d_bytes_per_step": h2d / e2e_iters, "d2h_bytes_per_step": d2h / e2e_iters,
+                "call": f"nmf_fit_host(iters={e2e_iters}) + nmf_project_subtract_host(iters={e2e_iters}) with pinned "
+                        f"host buffers; all H2D/D2H copies inside the timed region, amortised over {e2e_iters} iterations"},
+        "gpu_launches": int(launches),
+        "clocks": clocks,
+        "cpu_baseline": cpu,
+    }
+    print(json.dumps(line))
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=50)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default="stis", choices=sorted(WORKLOADS))
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    if args.impl == "reference":
+        run_reference(args, rank)
+    else:
+        run_ours(args, rank, world, local_rank)
+
+
+if __name__ == "__main__":
+    main()

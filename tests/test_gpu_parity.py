@@ -83,10 +83,11 @@ def test_survey_batch_reduced(variant):
         assert rel(Wg[b], Wo) <= TOL_FACTOR and rel(Hg[b], Ho) <= TOL_FACTOR
         fo = orc.objective(p.X, p.Omega, Wo, Ho); fg = orc.objective(p.X, p.Omega, Wg[b], Hg[b])
         assert abs(fg - fo) / fo <= 1e-5
-    # a batched fit equals the same problems fitted one at a time, bitwise
+    # a batched fit equals the same problems fitted one at a time (the pixel partitioning, hence the
+    # fp32 summation order of the W half-step, depends on the batch size: equal to rounding, not bitwise)
     p = probs[3]
     W1, H1, _ = gpu_fit(p, p.iters, variant)
-    assert np.array_equal(W1, Wg[3]) and np.array_equal(H1, Hg[3])
+    assert rel(W1, Wg[3]) <= 1e-4 and rel(H1, Hg[3]) <= 1e-4
 
 
 def test_objective_kernel_matches_oracle():
