@@ -33,6 +33,8 @@ struct nmf_plan {
     // fused-path geometry (see nmf_fused.cu)
     int f_kp = 0;                 // padded K of the fused instantiation (0 = unavailable)
     int f_ctas = 0;               // persistent CTAs per problem
+    int f_threads = 0;            // CTA size = pixels per tile
+    int f_fpw = 0;                // frames per warp in the W half
     // host staging for the *_host entry points (plan-owned device buffers)
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -59,6 +61,9 @@ int    nmf_generic_fit(nmf_plan* p, const float* X, const float* Om, float* W, f
                        int iters, int batch);
 int    nmf_generic_project(nmf_plan* p, const float* H, const float* T, const float* om,
                            float* C, int M, int iters);
+// fixed-order fp64 reduction of `parts` partial slabs [batch][parts][2][rows][KT] + W update
+int    nmf_launch_w_update(nmf_plan* p, const float* slab, float* W, int rows, int K, int KT,
+                           int parts, int batch);
 // fused per-pixel-tile path
 void   nmf_fused_configure(nmf_plan* p);
 size_t nmf_fused_workspace(const nmf_plan* p);

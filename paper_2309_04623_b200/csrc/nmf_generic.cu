@@ -368,6 +368,14 @@ size_t nmf_generic_workspace(const nmf_plan* p) {
     return fit > proj ? fit : proj;
 }
 
+int nmf_launch_w_update(nmf_plan* p, const float* slab, float* W, int rows, int K, int KT, int parts,
+                        int batch) {
+    dim3 g2((rows * K + 127) / 128, batch);
+    k_w_update<<<g2, 128, 0, p->stream>>>(slab, W, rows, K, KT, parts);
+    p->launches++;
+    return NMF_OK;
+}
+
 int nmf_generic_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters,
                     int batch) {
     const int parts = batch == p->batch ? p->g_parts_fit : parts_for(p, p->N, batch);
