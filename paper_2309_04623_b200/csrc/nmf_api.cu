@@ -10,7 +10,10 @@ inline bool misaligned(const void* p) { return (reinterpret_cast<uintptr_t>(p) &
 size_t plan_workspace(nmf_plan* p) {
     size_t g = nmf_generic_workspace(p);
     size_t f = nmf_fused_workspace(p);
-    size_t main = nmf_align_up(g > f ? g : f, 256);
+    size_t t = nmf_tc_workspace(p);
+    if (f > g) g = f;
+    if (t > g) g = t;
+    size_t main = nmf_align_up(g, 256);
     return main + nmf_align_up(nmf_aux_workspace(p), 256);
 }
 
@@ -19,9 +22,13 @@ int check_ws(const nmf_plan* p) {
     return NMF_OK;
 }
 
-bool use_fused(const nmf_plan* p) {
-    if (p->variant_req == 1) return false;
-    return nmf_fused_available(p);
+// 0 auto: tensor core > fused FFMA > generic
+int pick_variant(const nmf_plan* p) {
+    if (p->variant_req == 1) return 1;
+    if (p->variant_req == 2) return nmf_fused_available(p) ? 2 : 1;
+    if (nmf_tc_available(p)) return 3;
+    if (p->variant_req == 3) return 1;
+    return nmf_fused_available(p) ? 2 : 1;
 }
 
 int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
@@ -33,7 +40,10 @@ int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
     if (rc) return rc;
     if (iters == 0) return NMF_OK;
     if (p->variant_req == 2 && !nmf_fused_available(p)) return NMF_ERR_UNSUPPORTED;
-    if (use_fused(p)) return nmf_fused_fit(p, X, Om, W, H, iters, batch);
+    if (p->variant_req == 3 && !nmf_tc_available(p)) return NMF_ERR_UNSUPPORTED;
+    const int v = pick_variant(p);
+    if (v == 3) return nmf_tc_fit(p, X, Om, W, H, iters, batch);
+    if (v == 2) return nmf_fused_fit(p, X, Om, W, H, iters, batch);
     return nmf_generic_fit(p, X, Om, W, H, iters, batch);
 }
 
@@ -73,6 +83,7 @@ int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int ma
     p->device = dev; p->num_sms = prop.multiProcessorCount;
     nmf_generic_configure(p);
     nmf_fused_configure(p);
+    nmf_tc_configure(p);
     p->ws_needed = plan_workspace(p);
     *out = p;
     return NMF_OK;
@@ -95,14 +106,14 @@ int nmf_plan_set_stream(nmf_plan* p, void* s) {
 }
 
 int nmf_plan_set_variant(nmf_plan* p, int v) {
-    if (!p || v < 0 || v > 2) return NMF_ERR_INVALID_ARG;
+    if (!p || v < 0 || v > 3) return NMF_ERR_INVALID_ARG;
     p->variant_req = v;
     return NMF_OK;
 }
 
 int nmf_plan_get_variant(const nmf_plan* p) {
     if (!p) return NMF_ERR_INVALID_ARG;
-    return use_fused(p) ? 2 : 1;
+    return pick_variant(p);
 }
 
 int nmf_plan_destroy(nmf_plan* p) {

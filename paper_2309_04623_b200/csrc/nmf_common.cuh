@@ -21,7 +21,7 @@ struct nmf_plan {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     size_t ws_needed = 0;
-    int variant_req = 0;          // 0 auto, 1 generic, 2 fused
+    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 tensor core
     long long launches = 0;
     int sticky = 0;               // first CUDA error seen (nmf_status)
     std::string cuda_msg;
@@ -35,6 +35,10 @@ struct nmf_plan {
     int f_ctas = 0;               // persistent CTAs per problem
     int f_threads = 0;            // CTA size = pixels per tile
     int f_fpw = 0;                // frames per warp in the W half
+    // tensor-core path geometry (see nmf_tcfit.cu)
+    int t_ctas = 0;               // persistent CTAs per problem (0 = unavailable)
+    int t_nst = 0;                // cp.async sub-stage depth of the W phase
+    bool t_attr_done = false;
     // host staging for the *_host entry points (plan-owned device buffers)
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -70,6 +74,12 @@ size_t nmf_fused_workspace(const nmf_plan* p);
 bool   nmf_fused_available(const nmf_plan* p);
 int    nmf_fused_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
                      int iters, int batch);
+// tcgen05 tensor-core fused path (BF16x3 split, FP32 accumulation in TMEM)
+void   nmf_tc_configure(nmf_plan* p);
+size_t nmf_tc_workspace(const nmf_plan* p);
+bool   nmf_tc_available(const nmf_plan* p);
+int    nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
+                  int iters, int batch);
 // auxiliaries
 size_t nmf_aux_workspace(const nmf_plan* p);
 int    nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C,
