@@ -253,25 +253,42 @@ def run_ours(args, rank, world, local_rank):
         cpu = {"value": rate, "unit": UNIT, "cores": cores, "kind": "oracle",
                "sample": f"2 timed steps (+1 warm-up) on the first {crop_rows} image rows ({crop_rows * p.S} of {P} px) "
                          f"of all {N} frames, K={K}, {sec:.2f} s per crop step; rate scaled by the pixel fraction"}
+    roof_common = {"traffic": traffic, "algorithmic_flops_per_launch": F,
+                   "algorithmic_bytes_per_launch": bytes_per_iter(N, P, K),
+                   "hbm_time_floor_ms": bytes_per_iter(N, P, K) / (hbm_peak * 1e9) * 1e3,
+                   "hbm_peak_gbs_measured": hbm_peak,
+                   "achieved_gbs_algorithmic": bytes_per_iter(N, P, K) / (fit_ms_avg * 1e-3) / 1e9}
+    if plan.variant == 3:
+        # BF16x3: every FP32 product is six BF16 tensor-core products, so the pipe peak for
+        # the ALGORITHMIC 12NKP flops is the measured dense BF16 rate / 6 (sustained figure: the kernel is timed
+        # inside a multi-kernel step).
+        bf16 = peaks.get("bf16_tflops_sustained", 1400.0)
+        tpeak = bf16 / 6.0
+        roofline = {"bound": "tensor", "achieved": achieved, "peak": tpeak, "unit": "TFLOP/s", "frac": achieved / tpeak,
+                    "kernel": "fit iteration (k_tc_iter: tcgen05 BF16x3 fused tile kernel, + fixed-order reduce/W update)",
+                    "peak_source": (f"MEASURED_PEAKS.json bf16_tflops_sustained ({bf16}) / 6 piece products per FP32 product"
+                                    if peaks else "fallback 1400 TF/s sustained bf16 / 6"),
+                    "frac_of_ffma_roofline": achieved / ALU_PEAK_TFLOPS, **roof_common}
+    else:
+        roofline = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
+                    "frac": achieved / ALU_PEAK_TFLOPS,
+                    "kernel": "fit iteration (fused tile kernel + fixed-order reduce/W update)" if plan.variant == 2
+                              else "fit iteration (H half-step + W half-step partial + reduce kernels)",
+                    "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts/clocks)",
+                    **roof_common}
     line = {
         "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms_max / args.steps, "higher_is_better": True,
         "scaling": "weak", "vs_baseline": None, "dtype": "f32", "data": "synthetic",
         "config": {"workload": f"STIS-shaped N={N} {p.S}x{p.S}px K={K} M={M} (BASELINE.json configs[2])",
                    "step": "1 NMF iteration (a1-a8) + 1 projection iteration of M frames (a9) + subtraction (a10)",
-                   "fit_variant": {1: "generic two-kernel", 2: "fused per-pixel-tile"}[plan.variant],
+                   "fit_variant": {1: "generic two-kernel", 2: "fused per-pixel-tile FFMA",
+                                   3: "fused per-pixel-tile tcgen05 BF16x3"}[plan.variant],
                    "l2": "inputs (X+Omega 1.6 GB per step) are larger than the 126 MB L2; no explicit flush",
                    "parallelism": f"{world} independent replica(s), no collective"},
         "fit_ms_per_iter": fit_ms_avg,
         "fit_iterations_per_s": 1e3 / fit_ms_avg,
-        "roofline": {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
-                     "frac": achieved / ALU_PEAK_TFLOPS, "traffic": traffic,
-                     "kernel": "fit iteration (fused tile kernel + fixed-order reduce/W update)" if plan.variant == 2
-                               else "fit iteration (H half-step + W half-step partial + reduce kernels)",
-                     "algorithmic_flops_per_launch": F, "algorithmic_bytes_per_launch": bytes_per_iter(N, P, K),
-                     "peak_source": "derived: 148 SMs x 128 FP32 lanes x 2 x 1.965 GHz (B200_PROFILING.md unit counts/clocks)",
-                     "hbm_time_floor_ms": bytes_per_iter(N, P, K) / (hbm_peak * 1e9) * 1e3,
-                     "hbm_peak_gbs_measured": hbm_peak},
+        "roofline": roofline,
         "e2e": {"value": world * e2e_iters / e2e_s, "unit": UNIT,
                 "h2d_bytes_per_step": h2d / e2e_iters, "d2h_bytes_per_step": d2h / e2e_iters,
                 "call": f"nmf_fit_host(iters={e2e_iters}) + nmf_project_subtract_host(iters={e2e_iters}) with pinned "
@@ -290,7 +307,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="stis", choices=sorted(WORKLOADS))
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused FFMA, 3 tensor core")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup

@@ -13,7 +13,7 @@ from gpu_util import (TOL_FACTOR, check_fit_parity, check_project_subtract_parit
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [1, 0]   # 1 = generic two-kernel path, 0 = automatic (fused when available)
+VARIANTS = [1, 2, 0]   # 1 = generic two-kernel path, 2 = fused FFMA, 0 = automatic (tensor-core path when available)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)

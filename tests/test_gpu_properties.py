@@ -11,7 +11,7 @@ from paper_2309_04623_b200 import inputs, nmf
 from gpu_util import TOL_FACTOR, check_fit_parity, dev, gpu_fit, rel
 
 pytestmark = pytest.mark.gpu
-VARIANTS = [1, 0]
+VARIANTS = [1, 2, 0]   # generic, fused FFMA, automatic (tensor-core path when K <= 64)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -64,6 +64,8 @@ def test_power_of_two_homogeneity_bitwise(variant):
                                    (129, 2052, 33), (200, 996, 50), (256, 516, 128), (225, 260, 53)])
 def test_ragged_and_extreme_shapes(variant, N, P, K):
     """N, K, P off every tile size; K=1; the compiled maxima N=256, K=128; row-varying zeros in Omega."""
+    if variant == 2 and K > 50:
+        pytest.skip("the fused FFMA instantiations stop at K = 50")
     rng = np.random.default_rng(N * 1000 + K)
     X = (rng.random((N, P)) * 10).astype(np.float32)
     Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.25)).astype(np.float32)
