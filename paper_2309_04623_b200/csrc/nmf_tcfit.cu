@@ -1,54 +1,63 @@
 // nmf_tcfit.cu -- fused per-pixel-tile NMF iteration on the tcgen05 tensor cores.
 //
-// One persistent CTA (8 element-wise warps + 1 MMA-issuing warp) walks tiles of 128 pixels.  All six
-// contractions of Eq. 3 run as tcgen05.mma kind::f16 on BF16 operands with FP32
-// accumulation in TMEM.  Every FP32 operand x is split exactly into three BF16 pieces
-// x = x1 + x2 + x3 (x1 = bf16(x), x2 = bf16(x - x1), x3 = x - x1 - x2) and a product a*b is evaluated as
-// the six piece products a1b1 + a1b2 + a2b1 + a2b2 + a1b3 + a3b1 (dropped terms <= 2^-24 |ab|), so the
-// arithmetic stays FP32-faithful ("BF16x3", the BF16 analogue of the 3xTF32 split; it is used instead of
-// TF32 because 16-bit operands can be read both K-major and MN-major from one no-swizzle buffer, which
-// lets W and H' serve two contractions each from a single shared-memory copy).
+// One persistent, warp-specialised CTA per SM walks tiles of 128 pixels:
+//   warps 0-7  element-wise warps, two groups of four (one thread per TMEM lane in each group)
+//   warp  8    MMA issuer (one thread issues every tcgen05.mma / tcgen05.commit)
+//   warp  9    TMA producer (one thread streams H, X and Omega tiles through a ring of 16 KB slots)
+// All six contractions of Eq. 3 run as tcgen05.mma kind::f16 on BF16 operands with FP32
+// accumulation in TMEM.  Every FP32 operand x is split exactly into three BF16 pieces x = x1 + x2 + x3
+// (x1 = bf16(x), x2 = bf16(x - x1), x3 = x - x1 - x2) and a product a*b is evaluated as the six piece
+// products a1b1 + a1b2 + a2b1 + a2b2 + a1b3 + a3b1 (dropped terms <= 2^-24 |ab|), so the arithmetic stays
+// FP32-faithful ("BF16x3", the BF16 analogue of the 3xTF32 split; 16-bit operands can be read both K-major
+// and MN-major from one no-swizzle buffer, so W and H' serve two contractions each from one copy).
 //
 // Per tile (p0 .. p0+127), with W (3 pieces, [frames][comps]) resident in shared memory:
-//   H phase (TMEM lane = pixel):
-//     H0   the H tile is split and written to shared memory as Hs[pixel][comp]           (a1)
-//     S    S^T[pixel][frame] = Hs . Ws^T, 32 frames at a time (SS MMAs, N = 32)           (a2)
-//     EW   thread = (pixel, 16 frames): q = Om*X (select), r = Om*S, split -> TMEM        (a3)
-//     ND   Num^T += Q^T . W, Den^T += R^T . W   (A from TMEM, B = MN-major view of Ws)    (a4)
-//     UPD  h' = h * num / max(den, eps) -> global H and, split, back into Hs              (a5)
-//   W phase (TMEM lane = frame, two M tiles of 128 frames), 32 pixels at a time:
-//     S'   S'[frame][pixel] = Ws . Hs^T (SS MMAs, N = 32)                                 (a6)
-//     EW   thread = frame: X, Om re-read (L2) through cp.async-staged swizzled sub-tiles;
-//          q, r' = Om*S' split -> TMEM                                                    (a6)
+//   H phase (TMEM lane = pixel), 16 frames per chunk, chunk c handled by group c & 1:
+//     H0   the H tile (TMA -> ring) is split and written to shared memory as Hs[pixel][comp]       (a1)
+//     S    S^T[pixel][frame] = Hs . Ws^T  (SS MMAs, N = 16)                                         (a2)
+//     EW   thread = (pixel, 16 frames): X, Omega from the ring; q = Om*X (select), r = Om*S,
+//          split -> TMEM (R1, R2 overwrite S in place)                                              (a3)
+//     ND   Num^T += Q^T . W, Den^T += R^T . W   (A from TMEM, B = MN-major view of Ws)              (a4)
+//     UPD  h' = h * num / max(den, eps) -> global H and, split, back into Hs                        (a5)
+//   W phase (TMEM lane = frame, M tiles of 128 frames), 16 pixels per chunk, chunk c by group c & 1:
+//     S'   S'[frame][pixel] = Ws . Hs^T (SS MMAs, N = 16)                                           (a6)
+//     EW   thread = (frame, 16 pixels): X, Omega re-read (L2) through TMA (64-byte swizzled rows);
+//          q, r' = Om*S' split -> TMEM                                                              (a6)
 //     AB   A += Q . Hs, B += R' . Hs  (A from TMEM, B = MN-major view of Hs), accumulated in TMEM
-//          over all tiles of the CTA                                                      (a7)
+//          over all tiles of the CTA                                                                (a7)
 //   After the last tile the [2][N][64] accumulators go to this CTA's slab; nmf_launch_w_update reduces
 //   the slabs in fixed order and updates W (a8).
-// S / S' chunks are double-buffered in TMEM; the split pieces are single-buffered, so the element-wise
-// warps of chunk c+1 overlap the MMAs of chunk c except for their final piece stores.
+// Every chunk's S / piece columns are double-buffered in TMEM (one buffer per group), so the element-wise
+// work of chunk c+1 overlaps the MMAs of chunk c, and the TMA ring runs ahead across phase and tile borders.
+#include <cuda.h>
 #include "nmf_common.cuh"
 #include "nmf_tc.cuh"
 
 namespace {
 using namespace tc;
 
-constexpr int EW_THREADS = 256;            // warps 0..7
-constexpr int CTA_THREADS = 288;           // + warp 8 = MMA issuer
+constexpr int EW_WARPS = 8;
+constexpr int W_MMA = 8, W_TMA = 9;
+constexpr int CTA_THREADS = 320;
 constexpr int TILE = 128;                  // pixels per tile = UMMA M of the H phase
-constexpr int CHP = 32;                    // pixels per W-phase chunk
-constexpr int SUBP = 16;                   // pixels per cp.async sub-stage (64-byte rows)
+constexpr int FCH = 16;                    // frames per H-phase chunk (one UMMA K step)
+constexpr int PCH = 16;                    // pixels per W-phase chunk
+constexpr int NCH2 = TILE / PCH;           // W-phase chunks per tile
 constexpr int KP = 64;                     // components padded to the MN-major N of stages 2 and 4
 constexpr int HS_SB = 16 * 128;            // Hs: bytes between 8-component groups (128 pixels x 16 B)
 constexpr int HS_BYTES = 8 * HS_SB;        // one BF16 piece of the H tile
+constexpr int SLOT = 16384;                // ring slot bytes
+constexpr int MAX_SLOTS = 8;
 
-// TMEM columns (512 allocated)
-constexpr uint32_t T_S = 0;                // H phase: S_b at 32 b; R1/R2 overwrite it in place
-constexpr uint32_t T_R3 = 64;              //          R3 (+8 per k-step)
-constexpr uint32_t T_Q = 80;               //          Q_j at 16 j (+8 per k-step)
-constexpr uint32_t T_NUM = 128, T_DEN = 192;
-constexpr uint32_t T_S2 = 0;               // W phase: S'_b[m] at 64 b + 32 m
-constexpr uint32_t T_P2 = 128;             //          pieces[m] at 64 m: R'3 at +0, Q_j at 16 + 16 j
-constexpr uint32_t T_ACC = 256;            // A_acc[m] at 128 m, B_acc[m] at 128 m + 64
+// TMEM columns (512 allocated).  A super-chunk is two chunks (32 frames / 32 pixels), one per group.
+constexpr uint32_t T_NUM = 0, T_DEN = 64;  // H phase: Num^T, Den^T [pixel][64]
+constexpr uint32_t T_HZ = 128;             //   Z[jb] at T_HZ + 32 jb: S of super-chunk j (jb = j & 1); group g owns columns
+                                           //   16 g .. 16 g + 15 and overwrites them in place with R1 (8) and R2 (8)
+constexpr uint32_t T_HE = 192;             //   E[g] at T_HE + 32 g: R3, Q1, Q2, Q3 (8 columns each), single-buffered
+constexpr uint32_t T_WZ = 0;               // W phase: Z[jb][m] at 32 (2 jb + m)   (Num/Den are dead by then)
+constexpr uint32_t T_WE = 128;             //   E[g][m] at T_WE + 32 (2 g + m)
+constexpr uint32_t T_ACC = 256;            // A_acc[m] at T_ACC + 128 m, B_acc[m] at + 64 (persistent over tiles)
+constexpr uint32_t O_R3 = 0, O_Q1 = 8, O_Q2 = 16, O_Q3 = 24;   // inside an E buffer
 
 __host__ __device__ constexpr uint32_t idesc_bf16(int M, int N, int b_mn_major) {
     return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
@@ -64,12 +73,12 @@ __device__ __forceinline__ void mma16_ts(uint32_t d, uint32_t a, uint64_t b, uin
                  "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
                  ::"r"(d), "r"(a), "l"(b), "r"(id), "r"(acc) : "memory");
 }
+
 __device__ __forceinline__ bool elect_one() {
     uint32_t p;
     asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
     return p != 0;
 }
-__device__ __forceinline__ void named_bar_sync(int id, int n) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(n) : "memory"); }
 
 // exact 3-way BF16 split of two FP32 values, packed (low half = first value)
 __device__ __forceinline__ void split3_pair(float x0, float x1, uint32_t& p1, uint32_t& p2, uint32_t& p3) {
@@ -82,58 +91,91 @@ __device__ __forceinline__ void split3_pair(float x0, float x1, uint32_t& p1, ui
     asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(p3) : "f"(s1), "f"(s0));
 }
 
-__device__ __forceinline__ void cp_async16(uint32_t smem_dst, const void* gsrc, bool valid) {
-    const int sz = valid ? 16 : 0;                       // src-size 0: zero-fill, nothing is read
-    asm volatile("cp.async.cg.shared.global [%0], [%1], 16, %2;\n" ::"r"(smem_dst), "l"(gsrc), "r"(sz) : "memory");
+// q = Om*X, r = Om*S for 16 consecutive elements (Omega == 0: missing datum, skipped (G5); X may be NaN/Inf
+// there), split into BF16 pieces.  R1, R2 go back over S in place (`zcol`, this thread's lane); R3 and the Q pieces
+// are returned packed in `e` for the single-buffered E columns.
+__device__ __forceinline__ void ew16(const float (&x)[16], const float (&o)[16], const uint32_t (&s)[16], uint32_t zcol,
+                                     uint32_t (&e)[32]) {
+    uint32_t R1[8], R2[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float o0 = o[2 * i], o1 = o[2 * i + 1];
+        const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
+        const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
+        const float r0 = o0 > 0.f ? o0 * __uint_as_float(s[2 * i]) : 0.f;
+        const float r1 = o1 > 0.f ? o1 * __uint_as_float(s[2 * i + 1]) : 0.f;
+        split3_pair(q0, q1, e[O_Q1 + i], e[O_Q2 + i], e[O_Q3 + i]);
+        split3_pair(r0, r1, R1[i], R2[i], e[O_R3 + i]);
+    }
+    tmem_st8(zcol, R1); tmem_st8(zcol + 8, R2);
 }
-__device__ __forceinline__ void cp_async_commit() { asm volatile("cp.async.commit_group;\n" ::: "memory"); }
-template <int N_> __device__ __forceinline__ void cp_async_wait() { asm volatile("cp.async.wait_group %0;\n" ::"n"(N_) : "memory"); }
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
 
 struct TcArgs {
-    const float* X; const float* Om; const float* W; float* H; float* slab;
+    CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px]
+    CUtensorMap mXh, mOh;      // X, Om [B*N, P] box [16 frames][128 px]          (H phase)
+    CUtensorMap mXw, mOw;      // X, Om [B*N, P] box [N frames][16 px], 64-byte swizzle (W phase)
+    const float* W; float* H; float* slab;
     int N, K; long long P; long long n_tiles;
-    int NF;            // frames padded to a multiple of 32 (rows of the W pieces)
-    int MT;            // 128-frame M tiles of the W phase (1 or 2)
-    int KS;            // 16-component k-steps of stages 1 and 3
+    int NF;                    // frames padded to a multiple of 16 (rows of the W pieces)
+    int NC;                    // H-phase chunks = NF / 16
+    int MT;                    // 128-frame M tiles of the W phase (1 or 2)
+    int KH;                    // 32-component slots of the H tile (1 or 2)
+    int NS;                    // ring slots
 };
 
-// barrier slots
-enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P, B_ND, B_S20, B_S21, B_P2, B_ND2, B_COUNT };
+// mbarrier slots
+enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P0, B_P1, B_NDG0, B_NDG1, B_ND, B_S20, B_S21, B_P20, B_P21, B_ABG0, B_ABG1, B_AB,
+       B_FULL, B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
 
-template <int NST>
+template <int KS>
 __global__ void __launch_bounds__(CTA_THREADS, 1)
-k_tc_iter(const TcArgs g) {
+k_tc_iter(const __grid_constant__ TcArgs g) {
     extern __shared__ __align__(1024) unsigned char smem[];
-    const int N = g.N, K = g.K, NF = g.NF;
+    const int N = g.N, K = g.K, NF = g.NF, NC = g.NC, MT = g.MT, KH = g.KH;
+    const uint32_t NS = (uint32_t)g.NS;
     const long long P = g.P;
     const int WS_SB = (NF / 8) * 128;                   // Ws: bytes between 8-component groups
     const int WS_BYTES = 8 * WS_SB;
-    const int ST_ARR = N * (SUBP * 4);                  // one array (X or Om) of one sub-stage
     unsigned char* ws_p = smem;                         // 3 pieces of W
     unsigned char* hs_p = ws_p + 3 * WS_BYTES;          // 3 pieces of the H tile
-    unsigned char* stg = hs_p + 3 * HS_BYTES;           // NST sub-stages of {X, Om}
-    uint64_t* bars = reinterpret_cast<uint64_t*>(stg + (size_t)NST * 2 * ST_ARR);
+    unsigned char* ring = hs_p + 3 * HS_BYTES;          // NS slots of 16 KB (1024-byte aligned)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(ring + (size_t)NS * SLOT);
     uint32_t* tptr = reinterpret_cast<uint32_t*>(bars + B_COUNT);
 
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const int b = blockIdx.y;
-    const float* __restrict__ X = g.X + (size_t)b * N * P;
-    const float* __restrict__ Om = g.Om + (size_t)b * N * P;
     const float* __restrict__ W = g.W + (size_t)b * N * K;
     float* __restrict__ H = g.H + (size_t)b * K * P;
     float* slab = g.slab + ((size_t)b * gridDim.x + blockIdx.x) * 2 * (size_t)N * KP;
 
     // ---------------- setup: barriers, TMEM, W pieces ----------------
     if (tid == 0) {
-        mbar_init(&bars[B_HS], EW_THREADS); mbar_init(&bars[B_HS2], EW_THREADS);
+        mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_HS2], EW_WARPS);
         mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1);
-        mbar_init(&bars[B_P], EW_THREADS); mbar_init(&bars[B_ND], 1);
+        mbar_init(&bars[B_P0], 4); mbar_init(&bars[B_P1], 4); mbar_init(&bars[B_ND], 1);
+        mbar_init(&bars[B_NDG0], 1); mbar_init(&bars[B_NDG1], 1);
         mbar_init(&bars[B_S20], 1); mbar_init(&bars[B_S21], 1);
-        mbar_init(&bars[B_P2], EW_THREADS); mbar_init(&bars[B_ND2], 1);
+        mbar_init(&bars[B_P20], 4); mbar_init(&bars[B_P21], 4); mbar_init(&bars[B_AB], 1);
+        mbar_init(&bars[B_ABG0], 1); mbar_init(&bars[B_ABG1], 1);
+        for (uint32_t s = 0; s < NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 4); }
         mbar_fence_init();
     }
-    if (warp == 8) tmem_alloc(tptr, 512);
+    if (warp == W_MMA) tmem_alloc(tptr, 512);
+    if (warp == W_TMA && lane == 0) {
+        tma_prefetch_desc(&g.mH); tma_prefetch_desc(&g.mXh); tma_prefetch_desc(&g.mOh);
+        tma_prefetch_desc(&g.mXw); tma_prefetch_desc(&g.mOw);
+    }
     for (int i = tid; i < NF * 8; i += CTA_THREADS) {   // (frame n, component group kg): 8 values -> 3 x 16 B
         const int n = i >> 3, kg = i & 7;
         uint32_t p1[4], p2[4], p3[4];
@@ -154,219 +196,249 @@ k_tc_iter(const TcArgs g) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tptr;
-    const uint32_t ws_s = smem_u32(ws_p), hs_s = smem_u32(hs_p), stg_s = smem_u32(stg);
-    const int n_chunks = NF / 32;                       // H-phase chunks of 32 frames
-    constexpr int n_chunks2 = TILE / CHP;               // W-phase chunks of 32 pixels
-    constexpr int n_sub = TILE / SUBP;
-    constexpr int LOOK = NST - 1;
+    const uint32_t ws_s = smem_u32(ws_p), hs_s = smem_u32(hs_p), ring_s = smem_u32(ring);
+    const uint32_t slots_per_tile = (uint32_t)(KH + NC + 2 * NCH2);
 
-    if (warp == 8) {
-        // =========================== MMA issuer ===========================
-        uint32_t ph_hs = 0, ph_hs2 = 0, ph_p = 0, ph_p2 = 0;
-        uint32_t acc_started = 0;
-        const uint32_t id_s = idesc_bf16(128, 32, 0), id_nd = idesc_bf16(128, 64, 1);
-        // piece pairs (a, b), small products first: a1b3 a3b1 a2b2 a1b2 a2b1 a1b1
-        const int pa[6] = {0, 2, 1, 0, 1, 0}, pb[6] = {2, 0, 1, 1, 0, 0};
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
-            // ---- H phase ----
-            mbar_wait(&bars[B_HS], ph_hs); ph_hs ^= 1;
-            tc_fence_after();
-            for (int c = -1; c < n_chunks; ++c) {
-                if (c + 1 < n_chunks) {                  // S(c+1): [128 px] x [32 frames], K = comps
-                    if (elect_one()) {
-                        const int cc = c + 1;
-                        const uint32_t d = tmem + T_S + 32 * (cc & 1);
-                        uint32_t acc = 0;
-#pragma unroll
-                        for (int pr = 0; pr < 6; ++pr)
-                            for (int ks = 0; ks < g.KS; ++ks) {
-                                const uint64_t ad = smem_desc(hs_s + pa[pr] * HS_BYTES + ks * 2 * HS_SB, HS_SB, 128);
-                                const uint64_t bd = smem_desc(ws_s + pb[pr] * WS_BYTES + cc * 4 * 128 + ks * 2 * WS_SB, WS_SB, 128);
-                                mma16_ss(d, ad, bd, id_s, acc);
-                                acc = 1;
-                            }
-                        mma_commit(&bars[B_S0 + (cc & 1)]);
-                    }
-                    __syncwarp();
+    if (warp == W_TMA) {
+        // =========================== TMA producer ===========================
+        if (lane == 0) {
+            uint32_t seq = 0;
+            auto acquire = [&](uint32_t bytes) -> uint32_t {      // next ring slot, armed for `bytes`
+                const uint32_t s = seq % NS, par = (seq / NS) & 1u;
+                mbar_wait(&bars[B_EMPTY + s], par ^ 1u);
+                mbar_expect_tx(&bars[B_FULL + s], bytes);
+                ++seq;
+                return s;
+            };
+            for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+                const int p0 = (int)(tile * TILE);
+                for (int h = 0; h < KH; ++h) {
+                    const uint32_t s = acquire(32 * TILE * 4);
+                    tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
                 }
-                if (c >= 0) {                            // ND(c): Num^T, Den^T += pieces(c) . W
-                    mbar_wait(&bars[B_P], ph_p); ph_p ^= 1;
-                    tc_fence_after();
-                    if (elect_one()) {
-                        const uint32_t sb = tmem + T_S + 32 * (c & 1);
-#pragma unroll
-                        for (int ks = 0; ks < 2; ++ks) {
-                            const uint32_t a_q[3] = {tmem + T_Q + 8 * ks, tmem + T_Q + 16 + 8 * ks, tmem + T_Q + 32 + 8 * ks};
-                            const uint32_t a_r[3] = {sb + 16 * ks, sb + 16 * ks + 8, tmem + T_R3 + 8 * ks};
-                            const uint32_t frow = (uint32_t)(c * 4 + ks * 2) * 128;   // 16 frames = 2 row groups
-#pragma unroll
-                            for (int pr = 0; pr < 6; ++pr) {
-                                const uint64_t bd = smem_desc(ws_s + pb[pr] * WS_BYTES + frow, 128, WS_SB);
-                                const uint32_t acc = (c > 0 || ks > 0 || pr > 0) ? 1u : 0u;
-                                mma16_ts(tmem + T_NUM, a_q[pa[pr]], bd, id_nd, acc);
-                                mma16_ts(tmem + T_DEN, a_r[pa[pr]], bd, id_nd, acc);
-                            }
-                        }
-                        mma_commit(&bars[B_ND]);
-                    }
-                    __syncwarp();
+                for (int c = 0; c < NC; ++c) {
+                    const uint32_t s = acquire(2 * FCH * TILE * 4);
+                    tma_load_2d(ring_s + s * SLOT, &g.mXh, p0, b * N + FCH * c, &bars[B_FULL + s]);
+                    tma_load_2d(ring_s + s * SLOT + FCH * TILE * 4, &g.mOh, p0, b * N + FCH * c, &bars[B_FULL + s]);
                 }
-            }
-            // ---- W phase ----
-            mbar_wait(&bars[B_HS2], ph_hs2); ph_hs2 ^= 1;
-            tc_fence_after();
-            for (int c = -1; c < n_chunks2; ++c) {
-                if (c + 1 < n_chunks2) {                 // S'(c+1)[m]: [128 frames] x [32 px], K = comps
-                    if (elect_one()) {
-                        const int cc = c + 1;
-                        for (int m = 0; m < g.MT; ++m) {
-                            const uint32_t d = tmem + T_S2 + 64 * (cc & 1) + 32 * m;
-                            uint32_t acc = 0;
-#pragma unroll
-                            for (int pr = 0; pr < 6; ++pr)
-                                for (int ks = 0; ks < g.KS; ++ks) {
-                                    const uint64_t ad = smem_desc(ws_s + pa[pr] * WS_BYTES + m * 16 * 128 + ks * 2 * WS_SB, WS_SB, 128);
-                                    const uint64_t bd = smem_desc(hs_s + pb[pr] * HS_BYTES + cc * 4 * 128 + ks * 2 * HS_SB, HS_SB, 128);
-                                    mma16_ss(d, ad, bd, id_s, acc);
-                                    acc = 1;
-                                }
-                        }
-                        mma_commit(&bars[B_S20 + (cc & 1)]);
-                    }
-                    __syncwarp();
-                }
-                if (c >= 0) {                            // AB(c): A_acc += Q . Hs, B_acc += R' . Hs
-                    mbar_wait(&bars[B_P2], ph_p2); ph_p2 ^= 1;
-                    tc_fence_after();
-                    if (elect_one()) {
-                        for (int m = 0; m < g.MT; ++m) {
-                            const uint32_t sb = tmem + T_S2 + 64 * (c & 1) + 32 * m;
-                            const uint32_t pb2 = tmem + T_P2 + 64 * m;
-#pragma unroll
-                            for (int ks = 0; ks < 2; ++ks) {
-                                const uint32_t a_q[3] = {pb2 + 16 + 8 * ks, pb2 + 32 + 8 * ks, pb2 + 48 + 8 * ks};
-                                const uint32_t a_r[3] = {sb + 16 * ks, sb + 16 * ks + 8, pb2 + 8 * ks};
-                                const uint32_t prow = (uint32_t)(c * 4 + ks * 2) * 128;   // 16 pixels = 2 row groups
-#pragma unroll
-                                for (int pr = 0; pr < 6; ++pr) {
-                                    const uint64_t bd = smem_desc(hs_s + pb[pr] * HS_BYTES + prow, 128, HS_SB);
-                                    const uint32_t acc = (acc_started || ks > 0 || pr > 0) ? 1u : 0u;
-                                    mma16_ts(tmem + T_ACC + 128 * m, a_q[pa[pr]], bd, id_nd, acc);
-                                    mma16_ts(tmem + T_ACC + 128 * m + 64, a_r[pa[pr]], bd, id_nd, acc);
-                                }
-                            }
-                        }
-                        mma_commit(&bars[B_ND2]);
-                    }
-                    acc_started = 1;
-                    __syncwarp();
+                for (int c = 0; c < NCH2; ++c) {
+                    uint32_t s = acquire((uint32_t)N * PCH * 4);
+                    tma_load_2d(ring_s + s * SLOT, &g.mXw, p0 + PCH * c, b * N, &bars[B_FULL + s]);
+                    s = acquire((uint32_t)N * PCH * 4);
+                    tma_load_2d(ring_s + s * SLOT, &g.mOw, p0 + PCH * c, b * N, &bars[B_FULL + s]);
                 }
             }
         }
+    } else if (warp == W_MMA) {
+        // =========================== MMA issuer (whole warp converged; one elected lane issues) ===========================
+        uint32_t ph = 0;                              // phase bits, indexed by barrier slot
+        auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; tc_fence_after(); };
+        constexpr uint32_t id_s32 = idesc_bf16(128, 32, 0), id_s16 = idesc_bf16(128, 16, 0), id_nd = idesc_bf16(128, 64, 1);
+        // piece pairs (a, b), small products first: a1b3 a3b1 a2b2 a1b2 a2b1 a1b1
+        constexpr int pa[6] = {0, 2, 1, 0, 1, 0}, pb[6] = {2, 0, 1, 1, 0, 0};
+        uint64_t d_hs_k[3], d_hs_mn[3], d_ws_k[3], d_ws_mn[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            d_hs_k[i] = smem_desc(hs_s + i * HS_BYTES, HS_SB, 128);
+            d_hs_mn[i] = smem_desc(hs_s + i * HS_BYTES, 128, HS_SB);
+            d_ws_k[i] = smem_desc(ws_s + i * WS_BYTES, WS_SB, 128);
+            d_ws_mn[i] = smem_desc(ws_s + i * WS_BYTES, 128, WS_SB);
+        }
+        const uint32_t ws_kstep = (uint32_t)(2 * WS_SB) >> 4;
+        constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
+        const int NSC = (NC + 1) / 2;                    // H-phase super-chunks of 32 frames (the last may hold 16)
+        constexpr int NSC2 = NCH2 / 2;                   // W-phase super-chunks of 32 pixels
+        uint32_t acc_started = 0;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+            // ---- H phase ----
+            auto issue_S = [&](int j) {                  // S(j): [128 px] x [32 frames], K = comps -> Z[j & 1]
+                if (elect_one()) {
+                    const uint32_t d = tmem + T_HZ + 32 * (j & 1);
+                    const uint32_t boff = (uint32_t)(j * 4 * 128) >> 4;
+                    const uint32_t id = (2 * j + 1 < NC) ? id_s32 : id_s16;
+#pragma unroll
+                    for (int pr = 0; pr < 6; ++pr)
+#pragma unroll
+                        for (int ks = 0; ks < KS; ++ks)
+                            mma16_ss(d, d_hs_k[pa[pr]] + ks * hs_kstep, d_ws_k[pb[pr]] + boff + ks * ws_kstep, id,
+                                     (pr | ks) ? 1u : 0u);
+                    mma_commit(&bars[B_S0 + (j & 1)]);
+                }
+                __syncwarp();
+            };
+            wait(B_HS);
+            issue_S(0);
+            if (NSC > 1) issue_S(1);
+            for (int j = 0; j < NSC; ++j) {
+                for (int gg = 0; gg < 2; ++gg) {
+                    const int c = 2 * j + gg;
+                    if (c >= NC) break;
+                    wait(B_P0 + gg);
+                    if (elect_one()) {
+                        const uint32_t z = tmem + T_HZ + 32 * (j & 1) + 16 * gg, e = tmem + T_HE + 32 * gg;
+                        const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
+                        const uint32_t a_r[3] = {z, z + 8, e + O_R3};
+                        const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 frames = 2 row groups
+#pragma unroll
+                        for (int pr = 0; pr < 6; ++pr) {
+                            const uint32_t acc = (c > 0 || pr > 0) ? 1u : 0u;
+                            mma16_ts(tmem + T_NUM, a_q[pa[pr]], d_ws_mn[pb[pr]] + boff, id_nd, acc);
+                            mma16_ts(tmem + T_DEN, a_r[pa[pr]], d_ws_mn[pb[pr]] + boff, id_nd, acc);
+                        }
+                        mma_commit(&bars[B_NDG0 + gg]);
+                    }
+                    __syncwarp();
+                }
+                if (j + 2 < NSC) issue_S(j + 2);
+            }
+            if (elect_one()) mma_commit(&bars[B_ND]);
+            __syncwarp();
+            // ---- W phase ----
+            auto issue_S2 = [&](int j) {                 // S'(j)[m]: [128 frames] x [32 px], K = comps -> Z[j & 1][m]
+                if (elect_one()) {
+                    const uint32_t boff = (uint32_t)(j * 4 * 128) >> 4;
+                    for (int m = 0; m < MT; ++m) {
+                        const uint32_t d = tmem + T_WZ + 32 * (2 * (j & 1) + m);
+                        const uint32_t aoff = (uint32_t)(m * 16 * 128) >> 4;
+#pragma unroll
+                        for (int pr = 0; pr < 6; ++pr)
+#pragma unroll
+                            for (int ks = 0; ks < KS; ++ks)
+                                mma16_ss(d, d_ws_k[pa[pr]] + aoff + ks * ws_kstep, d_hs_k[pb[pr]] + boff + ks * hs_kstep,
+                                         id_s32, (pr | ks) ? 1u : 0u);
+                    }
+                    mma_commit(&bars[B_S20 + (j & 1)]);
+                }
+                __syncwarp();
+            };
+            wait(B_HS2);
+            issue_S2(0);
+            issue_S2(1);
+            for (int j = 0; j < NSC2; ++j) {
+                for (int gg = 0; gg < 2; ++gg) {
+                    const int c = 2 * j + gg;
+                    wait(B_P20 + gg);
+                    if (elect_one()) {
+                        const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
+                        for (int m = 0; m < MT; ++m) {
+                            const uint32_t z = tmem + T_WZ + 32 * (2 * (j & 1) + m) + 16 * gg;
+                            const uint32_t e = tmem + T_WE + 32 * (2 * gg + m);
+                            const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
+                            const uint32_t a_r[3] = {z, z + 8, e + O_R3};
+#pragma unroll
+                            for (int pr = 0; pr < 6; ++pr) {
+                                const uint32_t acc = (acc_started || pr > 0) ? 1u : 0u;
+                                mma16_ts(tmem + T_ACC + 128 * m, a_q[pa[pr]], d_hs_mn[pb[pr]] + boff, id_nd, acc);
+                                mma16_ts(tmem + T_ACC + 128 * m + 64, a_r[pa[pr]], d_hs_mn[pb[pr]] + boff, id_nd, acc);
+                            }
+                        }
+                        mma_commit(&bars[B_ABG0 + gg]);
+                    }
+                    __syncwarp();
+                    acc_started = 1;
+                }
+                if (j + 2 < NSC2) issue_S2(j + 2);
+            }
+            if (elect_one()) mma_commit(&bars[B_AB]);
+            __syncwarp();
+        }
     } else {
         // =========================== element-wise warps ===========================
-        const int q = warp & 3, half = warp >> 2;
+        const int q = warp & 3, grp = warp >> 2;
+        const int t = 32 * q + lane;                     // TMEM lane: H-phase pixel / W-phase frame in the M tile
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
-        uint32_t ph_s[2] = {0, 0}, ph_nd = 0, ph_s2[2] = {0, 0}, ph_nd2 = 0;
-        const int t = 32 * q + lane;                     // H phase: pixel within the tile
-        const int fr = 128 * half + 32 * q + lane;       // W phase: frame
-        const bool fr_ok = fr < N;
-        const bool do_tm = half < g.MT;
-
-        auto issue_sub = [&](long long p0, int s) {      // cp.async sub-stage s of the tile at p0
-            if (s < n_sub) {
-                const uint32_t dstb = stg_s + (uint32_t)(s % NST) * 2 * ST_ARR;
-                const long long ps = p0 + (long long)s * SUBP;
-                for (int i = tid; i < N * 4; i += EW_THREADS) {
-                    const int row = i >> 2, ch = i & 3;
-                    const long long p = ps + 4 * ch;
-                    const bool ok = p < P;               // P % 4 == 0: a chunk is all in or all out
-                    const size_t gi = (size_t)row * P + (ok ? p : 0);
-                    const uint32_t d = dstb + row * 64 + ((ch ^ ((row >> 1) & 3)) << 4);
-                    cp_async16(d, X + gi, ok);
-                    cp_async16(d + ST_ARR, Om + gi, ok);
-                }
-            }
-            cp_async_commit();
+        uint32_t ph = 0;
+        auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; };
+        auto wait_full = [&](uint32_t seq) -> const unsigned char* {
+            const uint32_t s = seq % NS;
+            mbar_wait(&bars[B_FULL + s], (seq / NS) & 1u);
+            return ring + (size_t)s * SLOT;
         };
+        auto release = [&](uint32_t seq) {               // this warp is done reading the slot
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[B_EMPTY + seq % NS]);
+        };
+        auto warp_arrive = [&](int bar) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[bar]);
+        };
+        uint32_t sq = 0;                                 // ring sequence number of this tile's first slot
+        bool first = true;
+        const int NSC = (NC + 1) / 2;
+        constexpr int NSC2 = NCH2 / 2;
 
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
-            const long long p0 = tile * TILE;
-            const long long p = p0 + t;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
+            const long long p = tile * TILE + t;
             const bool p_ok = p < P;
             const long long pc = p_ok ? p : P - 1;
-            named_bar_sync(1, EW_THREADS);               // every reader of the previous tile's stages is done
-#pragma unroll
-            for (int s = 0; s < LOOK; ++s) issue_sub(p0, s);
 
-            // ---- H0: split the H tile into Hs[pixel][comp] ----
+            // ---- H0: this group's 32 components of the H tile: keep h, split into Hs[pixel][comp] ----
+            float h[32];
+            if (grp < KH) {
+                const float* hsl = reinterpret_cast<const float*>(wait_full(sq + grp));
+#pragma unroll
+                for (int j = 0; j < 32; ++j) h[j] = (32 * grp + j < K) ? hsl[j * TILE + t] : 0.f;   // px >= P: zero-filled
+                release(sq + grp);
+            } else {
+#pragma unroll
+                for (int j = 0; j < 32; ++j) h[j] = 0.f;
+            }
+            if (!first) { wait(B_AB); }                  // every MMA of the previous tile is complete: Hs is free
+            first = false;
 #pragma unroll
             for (int gq = 0; gq < 4; ++gq) {
-                const int kg = 4 * half + gq;
                 uint32_t p1[4], p2[4], p3[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int k0 = kg * 8 + 2 * j;
-                    const float h0 = (p_ok && k0 < K) ? H[(size_t)k0 * P + pc] : 0.f;
-                    const float h1 = (p_ok && k0 + 1 < K) ? H[(size_t)(k0 + 1) * P + pc] : 0.f;
-                    split3_pair(h0, h1, p1[j], p2[j], p3[j]);
-                }
-                const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + kg * HS_SB;
+                for (int j = 0; j < 4; ++j) split3_pair(h[8 * gq + 2 * j], h[8 * gq + 2 * j + 1], p1[j], p2[j], p3[j]);
+                const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + (4 * grp + gq) * HS_SB;
                 *reinterpret_cast<uint4*>(hs_p + off) = make_uint4(p1[0], p1[1], p1[2], p1[3]);
                 *reinterpret_cast<uint4*>(hs_p + HS_BYTES + off) = make_uint4(p2[0], p2[1], p2[2], p2[3]);
                 *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(p3[0], p3[1], p3[2], p3[3]);
             }
             fence_proxy_async();
-            mbar_arrive(&bars[B_HS]);
+            warp_arrive(B_HS);
 
-            // ---- H phase chunks: thread = (pixel t, 16 frames) ----
-            for (int c = 0; c < n_chunks; ++c) {
-                const int bb = c & 1;
-                const int f0 = 32 * c + 16 * half;
+            // ---- H phase: super-chunk j = chunks 2j (group 0) and 2j + 1 (group 1); thread = (pixel t, 16 frames) ----
+            bool pending = false;                        // an ND of this group may still be reading E[grp]
+            for (int j = 0; j < NSC; ++j) {
+                const int c = 2 * j + grp;
+                const bool have = c < NC;
                 float x[16], o[16];
+                if (have) {
+                    const uint32_t seq = sq + KH + c;
+                    const float* xs = reinterpret_cast<const float*>(wait_full(seq));
+                    const int nv = N - FCH * c;          // valid frames of this chunk (>= 16: all)
 #pragma unroll
-                for (int i = 0; i < 16; ++i) {
-                    const int n = f0 + i;
-                    const bool ok = p_ok && n < N;
-                    o[i] = ok ? __ldg(Om + (size_t)n * P + pc) : 0.f;
-                    x[i] = ok ? __ldg(X + (size_t)n * P + pc) : 0.f;
+                    for (int i = 0; i < 16; ++i) {
+                        x[i] = xs[i * TILE + t];
+                        o[i] = i < nv ? xs[FCH * TILE + i * TILE + t] : 0.f;
+                    }
+                    release(seq);
                 }
-                mbar_wait(&bars[B_S0 + bb], ph_s[bb]); ph_s[bb] ^= 1;
-                tc_fence_after();
-                uint32_t s[16];
-                const uint32_t s_addr = lane_base + T_S + 32 * bb + 16 * half;
-                tmem_ld16(s_addr, s);
-                tmem_wait_ld();
-                uint32_t R1[8], R2[8], R3[8], Q1[8], Q2[8], Q3[8];
-#pragma unroll
-                for (int i = 0; i < 8; ++i) {
-                    const float o0 = o[2 * i], o1 = o[2 * i + 1];
-                    // Omega == 0: missing datum, skipped (G5); X may be NaN/Inf there
-                    const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
-                    const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
-                    const float r0 = o0 > 0.f ? o0 * __uint_as_float(s[2 * i]) : 0.f;
-                    const float r1 = o1 > 0.f ? o1 * __uint_as_float(s[2 * i + 1]) : 0.f;
-                    split3_pair(q0, q1, Q1[i], Q2[i], Q3[i]);
-                    split3_pair(r0, r1, R1[i], R2[i], R3[i]);
+                wait(B_S0 + (j & 1));                    // both groups track every completion of the buffer's barrier
+                if (have) {
+                    tc_fence_after();
+                    const uint32_t zcol = lane_base + T_HZ + 32 * (j & 1) + 16 * grp;
+                    uint32_t s[16], e[32];
+                    tmem_ld16(zcol, s);
+                    tmem_wait_ld();
+                    ew16(x, o, s, zcol, e);
+                    if (pending) { wait(B_NDG0 + grp); tc_fence_after(); }
+                    tmem_st32(lane_base + T_HE + 32 * grp, e);
+                    tmem_wait_st();
+                    tc_fence_before();
+                    warp_arrive(B_P0 + grp);
+                    pending = true;
                 }
-                tmem_st8(s_addr, R1);
-                tmem_st8(s_addr + 8, R2);
-                if (c > 0) { mbar_wait(&bars[B_ND], ph_nd); ph_nd ^= 1; tc_fence_after(); }
-                tmem_st8(lane_base + T_R3 + 8 * half, R3);
-                tmem_st8(lane_base + T_Q + 8 * half, Q1);
-                tmem_st8(lane_base + T_Q + 16 + 8 * half, Q2);
-                tmem_st8(lane_base + T_Q + 32 + 8 * half, Q3);
-                tmem_wait_st();
-                tc_fence_before();
-                mbar_arrive(&bars[B_P]);
             }
-            mbar_wait(&bars[B_ND], ph_nd); ph_nd ^= 1;   // Num, Den complete; every stage-1 read of Hs is done
+            if (pending) wait(B_NDG0 + grp);
+            wait(B_ND);                                  // Num, Den complete; every stage-1 read of Hs is done
             tc_fence_after();
 
-            // ---- UPD: h' = h * num / max(den, eps); thread = (pixel t, 32 comps) ----
+            // ---- UPD: h' = h * num / max(den, eps); thread = (pixel t, this group's 32 comps) ----
 #pragma unroll
             for (int gq = 0; gq < 4; ++gq) {
-                const int kg = 4 * half + gq;
+                const int kg = 4 * grp + gq;
                 uint32_t nm[8], dn[8];
                 tmem_ld8(lane_base + T_NUM + 8 * kg, nm);
                 tmem_ld8(lane_base + T_DEN + 8 * kg, dn);
@@ -377,8 +449,7 @@ k_tc_iter(const TcArgs g) {
                     const int k = kg * 8 + j;
                     float v = 0.f;
                     if (p_ok && k < K) {
-                        const float h = H[(size_t)k * P + pc];
-                        v = (h * __uint_as_float(nm[j])) / fmaxf(__uint_as_float(dn[j]), NMF_EPS);
+                        v = (h[8 * gq + j] * __uint_as_float(nm[j])) / fmaxf(__uint_as_float(dn[j]), NMF_EPS);
                         H[(size_t)k * P + pc] = v;
                     }
                     hn[j] = v;
@@ -393,31 +464,26 @@ k_tc_iter(const TcArgs g) {
             }
             fence_proxy_async();
             tc_fence_before();
-            mbar_arrive(&bars[B_HS2]);
+            warp_arrive(B_HS2);
 
-            // ---- W phase chunks: thread = frame, 2 x 16 pixels per chunk ----
-            for (int c = 0; c < n_chunks2; ++c) {
-                const int bb = c & 1;
-#pragma unroll
-                for (int hh = 0; hh < 2; ++hh) {
-                    const int s_idx = 2 * c + hh;
-                    cp_async_wait<LOOK - 1>();
-                    named_bar_sync(1, EW_THREADS);
-                    issue_sub(p0, s_idx + LOOK);
-                    if (hh == 0) { mbar_wait(&bars[B_S20 + bb], ph_s2[bb]); ph_s2[bb] ^= 1; tc_fence_after(); }
-                    uint32_t R1[8], R2[8], R3[8], Q1[8], Q2[8], Q3[8];
-                    const uint32_t s_addr = lane_base + T_S2 + 64 * bb + 32 * half + 16 * hh;
-                    if (do_tm) {
-                        uint32_t s[16];
-                        tmem_ld16(s_addr, s);
-                        float x[16], o[16];
-                        if (fr_ok) {
-                            const unsigned char* xr = stg + (size_t)(s_idx % NST) * 2 * ST_ARR + fr * 64;
+            // ---- W phase: super-chunk j = chunks 2j + grp; thread = (frames t and 128 + t, 16 pixels) ----
+            pending = false;
+            for (int j = 0; j < NSC2; ++j) {
+                const int c = 2 * j + grp;
+                const uint32_t seq = sq + KH + NC + 2 * c;
+                const unsigned char* xsl = wait_full(seq);
+                const unsigned char* osl = wait_full(seq + 1);
+                for (int m = 0; m < MT; ++m) {
+                    const int fr = 128 * m + t;
+                    const bool active = 128 * m + 32 * q < N;        // warp-uniform: some lane has a frame
+                    float x[16], o[16];
+                    if (active) {
+                        if (fr < N) {
                             const int sw = (fr >> 1) & 3;
 #pragma unroll
                             for (int ch = 0; ch < 4; ++ch) {
-                                const float4 xv = *reinterpret_cast<const float4*>(xr + ((ch ^ sw) << 4));
-                                const float4 ov = *reinterpret_cast<const float4*>(xr + ST_ARR + ((ch ^ sw) << 4));
+                                const float4 xv = *reinterpret_cast<const float4*>(xsl + fr * 64 + ((ch ^ sw) << 4));
+                                const float4 ov = *reinterpret_cast<const float4*>(osl + fr * 64 + ((ch ^ sw) << 4));
                                 x[4 * ch] = xv.x; x[4 * ch + 1] = xv.y; x[4 * ch + 2] = xv.z; x[4 * ch + 3] = xv.w;
                                 o[4 * ch] = ov.x; o[4 * ch + 1] = ov.y; o[4 * ch + 2] = ov.z; o[4 * ch + 3] = ov.w;
                             }
@@ -425,47 +491,41 @@ k_tc_iter(const TcArgs g) {
 #pragma unroll
                             for (int i = 0; i < 16; ++i) { x[i] = 0.f; o[i] = 0.f; }
                         }
+                    }
+                    if (m == MT - 1) { release(seq); release(seq + 1); }
+                    if (m == 0) { wait(B_S20 + (j & 1)); tc_fence_after(); }
+                    uint32_t e[32];
+                    if (active) {
+                        const uint32_t zcol = lane_base + T_WZ + 32 * (2 * (j & 1) + m) + 16 * grp;
+                        uint32_t s[16];
+                        tmem_ld16(zcol, s);
                         tmem_wait_ld();
-#pragma unroll
-                        for (int i = 0; i < 8; ++i) {
-                            const float o0 = o[2 * i], o1 = o[2 * i + 1];
-                            const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
-                            const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
-                            const float r0 = o0 > 0.f ? o0 * __uint_as_float(s[2 * i]) : 0.f;
-                            const float r1 = o1 > 0.f ? o1 * __uint_as_float(s[2 * i + 1]) : 0.f;
-                            split3_pair(q0, q1, Q1[i], Q2[i], Q3[i]);
-                            split3_pair(r0, r1, R1[i], R2[i], R3[i]);
-                        }
-                        tmem_st8(s_addr, R1);
-                        tmem_st8(s_addr + 8, R2);
+                        ew16(x, o, s, zcol, e);
                     }
-                    if (hh == 0 && c > 0) { mbar_wait(&bars[B_ND2], ph_nd2); ph_nd2 ^= 1; tc_fence_after(); }
-                    if (do_tm) {
-                        const uint32_t pbase = lane_base + T_P2 + 64 * half + 8 * hh;
-                        tmem_st8(pbase, R3);
-                        tmem_st8(pbase + 16, Q1);
-                        tmem_st8(pbase + 32, Q2);
-                        tmem_st8(pbase + 48, Q3);
-                    }
+                    if (m == 0 && pending) { wait(B_ABG0 + grp); tc_fence_after(); }
+                    if (active) tmem_st32(lane_base + T_WE + 32 * (2 * grp + m), e);
                 }
-                if (do_tm) tmem_wait_st();
+                tmem_wait_st();
                 tc_fence_before();
-                mbar_arrive(&bars[B_P2]);
+                warp_arrive(B_P20 + grp);
+                pending = true;
             }
-            mbar_wait(&bars[B_ND2], ph_nd2); ph_nd2 ^= 1;   // every MMA of this tile is complete
-            tc_fence_after();
-            cp_async_wait<0>();
+            wait(B_ABG0 + grp);
         }
+        wait(B_AB);                                      // every MMA of the last tile is complete
+        tc_fence_after();
 
         // ---- the CTA's accumulators -> its slab [2][N][KP] (grid <= n_tiles: every CTA had a tile) ----
-        if (do_tm) {
+        if (grp < MT) {
+            const int fr = 128 * grp + t;
+            const bool fr_ok = fr < N;
             float* sa = slab + (size_t)(fr_ok ? fr : 0) * KP;
             float* sb = sa + (size_t)N * KP;
 #pragma unroll
             for (int cg = 0; cg < 4; ++cg) {
                 uint32_t a[16], bq[16];
-                tmem_ld16(lane_base + T_ACC + 128 * half + 16 * cg, a);       // warp-collective: no lane predicate
-                tmem_ld16(lane_base + T_ACC + 128 * half + 64 + 16 * cg, bq);
+                tmem_ld16(lane_base + T_ACC + 128 * grp + 16 * cg, a);       // warp-collective: no lane predicate
+                tmem_ld16(lane_base + T_ACC + 128 * grp + 64 + 16 * cg, bq);
                 tmem_wait_ld();
                 if (fr_ok) {
 #pragma unroll
@@ -479,11 +539,53 @@ k_tc_iter(const TcArgs g) {
     }
     tc_fence_before();
     __syncthreads();
-    if (warp == 8) tmem_dealloc(tmem, 512);
+    if (warp == W_MMA) tmem_dealloc(tmem, 512);
 }
 
-size_t tc_smem(int N, int NF, int nst) {
-    return (size_t)3 * NF * 128 + 3 * HS_BYTES + (size_t)nst * 2 * N * SUBP * 4 + B_COUNT * 8 + 16;
+constexpr size_t SMEM_MAX = 227 * 1024;
+
+size_t tc_smem_fixed(int NF) { return (size_t)3 * NF * 128 + 3 * HS_BYTES + B_COUNT * 8 + 16; }
+
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency)
+typedef CUresult (*encode_fn_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+encode_fn_t encode_fn() {
+    static encode_fn_t fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<encode_fn_t>(p);
+    }
+    return fn;
+}
+
+// 2-D fp32 map over a row-major [rows, P] array, box [box_rows][box_px]
+bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, int box_rows, int box_px, bool swizzle64) {
+    encode_fn_t fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)P, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)P * sizeof(float)};
+    const cuuint32_t box[2] = {(cuuint32_t)box_px, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
+}
+
+template <int KS>
+cudaError_t launch_ks(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st) {
+    static bool attr_done = false;
+    if (!attr_done) {
+        cudaError_t e = cudaFuncSetAttribute(k_tc_iter<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+        if (e != cudaSuccess) return e;
+        attr_done = true;
+    }
+    k_tc_iter<KS><<<grid, CTA_THREADS, smem, st>>>(a);
+    return cudaSuccess;
 }
 
 }  // namespace
@@ -491,17 +593,18 @@ size_t tc_smem(int N, int NF, int nst) {
 void nmf_tc_configure(nmf_plan* p) {
     p->t_ctas = 0; p->t_nst = 0;
     if (p->K > KP || p->N > 256) return;
-    const int NF = (p->N + 31) / 32 * 32;
-    int nst = 3;
-    if (tc_smem(p->N, NF, nst) > 227 * 1024) nst = 2;
-    if (tc_smem(p->N, NF, nst) > 227 * 1024) return;
+    if (p->P + TILE >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
+    const int NF = (p->N + FCH - 1) / FCH * FCH;
+    long long ns = ((long long)SMEM_MAX - (long long)tc_smem_fixed(NF)) / SLOT;
+    if (ns > MAX_SLOTS) ns = MAX_SLOTS;
+    if (ns < 4) return;
     const long long n_tiles = (p->P + TILE - 1) / TILE;
     long long ctas = p->num_sms / p->batch;
     if (ctas < 1) ctas = 1;
     if (ctas > n_tiles) ctas = n_tiles;
     const long long per = (n_tiles + ctas - 1) / ctas;      // even out: every CTA gets `per` or one fewer
     ctas = (n_tiles + per - 1) / per;
-    p->t_ctas = (int)ctas; p->t_nst = nst;
+    p->t_ctas = (int)ctas; p->t_nst = (int)ns;
 }
 
 size_t nmf_tc_workspace(const nmf_plan* p) {
@@ -514,19 +617,29 @@ bool nmf_tc_available(const nmf_plan* p) { return p->t_ctas != 0; }
 int nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
     if (!p->t_ctas) return NMF_ERR_UNSUPPORTED;
     TcArgs a;
-    a.X = X; a.Om = Om; a.W = W; a.H = H; a.slab = reinterpret_cast<float*>(p->ws);
-    a.N = p->N; a.K = p->K; a.P = p->P; a.n_tiles = (p->P + TILE - 1) / TILE;
-    a.NF = (p->N + 31) / 32 * 32; a.MT = (p->N + 127) / 128; a.KS = (p->K + 15) / 16;
-    const size_t smem = tc_smem(p->N, a.NF, p->t_nst);
-    if (!p->t_attr_done) {
-        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_tc_iter<3>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_tc_iter<2>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        p->t_attr_done = true;
+    const long long rows = (long long)batch * p->N;
+    if (!make_map(&a.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) ||
+        !make_map(&a.mXh, X, rows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om, rows, p->P, FCH, TILE, false) ||
+        !make_map(&a.mXw, X, rows, p->P, p->N, PCH, true) || !make_map(&a.mOw, Om, rows, p->P, p->N, PCH, true)) {
+        if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
+        return NMF_ERR_CUDA;
     }
+    a.W = W; a.H = H; a.slab = reinterpret_cast<float*>(p->ws);
+    a.N = p->N; a.K = p->K; a.P = p->P; a.n_tiles = (p->P + TILE - 1) / TILE;
+    a.NF = (p->N + FCH - 1) / FCH * FCH; a.NC = a.NF / FCH; a.MT = (p->N + 127) / 128;
+    a.KH = (p->K + 31) / 32; a.NS = p->t_nst;
+    const int KS = (p->K + 15) / 16;
+    const size_t smem = tc_smem_fixed(a.NF) + (size_t)a.NS * SLOT;
     const dim3 grid(p->t_ctas, batch);
     for (int it = 0; it < iters; ++it) {
-        if (p->t_nst == 3) k_tc_iter<3><<<grid, CTA_THREADS, smem, p->stream>>>(a);
-        else k_tc_iter<2><<<grid, CTA_THREADS, smem, p->stream>>>(a);
+        cudaError_t e;
+        switch (KS) {
+            case 1: e = launch_ks<1>(a, grid, smem, p->stream); break;
+            case 2: e = launch_ks<2>(a, grid, smem, p->stream); break;
+            case 3: e = launch_ks<3>(a, grid, smem, p->stream); break;
+            default: e = launch_ks<4>(a, grid, smem, p->stream); break;
+        }
+        NMF_CUDA_TRY(p, e);
         p->launches++;
         int rc = nmf_launch_w_update(p, a.slab, W, p->N, p->K, KP, p->t_ctas, batch);
         if (rc) return rc;
