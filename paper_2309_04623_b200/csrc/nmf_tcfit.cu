@@ -80,15 +80,22 @@ __device__ __forceinline__ bool elect_one() {
     return p != 0;
 }
 
-// exact 3-way BF16 split of two FP32 values, packed (low half = first value)
+// exact 3-way BF16 split of two FP32 values, packed (low half = first value): x = x1 + x2 + x3 with
+// x1 = x rounded to 8 significant bits (half away from zero), x2 = the next 8 bits of the remainder (truncated),
+// x3 = what is left (at most 8 significant bits, so it is a BF16 number).  Integer / FADD / PRMT only: the
+// F2FP conversion pipe is a quarter-rate unit and was the limiter of the element-wise warps.
 __device__ __forceinline__ void split3_pair(float x0, float x1, uint32_t& p1, uint32_t& p2, uint32_t& p3) {
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(p1) : "f"(x1), "f"(x0));
-    const float r0 = x0 - __uint_as_float(p1 << 16);
-    const float r1 = x1 - __uint_as_float(p1 & 0xffff0000u);
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(p2) : "f"(r1), "f"(r0));
-    const float s0 = r0 - __uint_as_float(p2 << 16);
-    const float s1 = r1 - __uint_as_float(p2 & 0xffff0000u);
-    asm("cvt.rn.bf16x2.f32 %0, %1, %2;" : "=r"(p3) : "f"(s1), "f"(s0));
+    const uint32_t a0 = (__float_as_uint(x0) + 0x8000u) & 0xffff0000u;
+    const uint32_t a1 = (__float_as_uint(x1) + 0x8000u) & 0xffff0000u;
+    const float r0 = x0 - __uint_as_float(a0);
+    const float r1 = x1 - __uint_as_float(a1);
+    const uint32_t b0 = __float_as_uint(r0) & 0xffff0000u;
+    const uint32_t b1 = __float_as_uint(r1) & 0xffff0000u;
+    const float s0 = r0 - __uint_as_float(b0);
+    const float s1 = r1 - __uint_as_float(b1);
+    p1 = __byte_perm(a0, a1, 0x7632);
+    p2 = __byte_perm(b0, b1, 0x7632);
+    p3 = __byte_perm(__float_as_uint(s0), __float_as_uint(s1), 0x7632);
 }
 
 // q = Om*X, r = Om*S for 16 consecutive elements (Omega == 0: missing datum, skipped (G5); X may be NaN/Inf
@@ -102,8 +109,8 @@ __device__ __forceinline__ void ew16(const float (&x)[16], const float (&o)[16],
         const float o0 = o[2 * i], o1 = o[2 * i + 1];
         const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
         const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
-        const float r0 = o0 > 0.f ? o0 * __uint_as_float(s[2 * i]) : 0.f;
-        const float r1 = o1 > 0.f ? o1 * __uint_as_float(s[2 * i + 1]) : 0.f;
+        const float r0 = o0 * __uint_as_float(s[2 * i]);          // S is finite: Omega == 0 gives exactly 0
+        const float r1 = o1 * __uint_as_float(s[2 * i + 1]);
         split3_pair(q0, q1, e[O_Q1 + i], e[O_Q2 + i], e[O_Q3 + i]);
         split3_pair(r0, r1, R1[i], R2[i], e[O_R3 + i]);
     }
@@ -119,6 +126,19 @@ __device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32
           "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
         : "memory");
 }
+
+#ifdef NMF_TC_TRACE
+// diagnostic timeline (built only with -DNMF_TC_TRACE): (tag, clock64) pairs of CTA 0's third tile
+__device__ long long nmf_tc_trace_buf[3][1024];
+#define TR_DECL int tr_n = 0; int tr_tile = 0;
+#define TR(role, tag) do { if (blockIdx.x == 0 && blockIdx.y == 0 && tr_tile == 2 && lane == 0 && tr_n < 510) { \
+        nmf_tc_trace_buf[role][2 * tr_n] = (tag); nmf_tc_trace_buf[role][2 * tr_n + 1] = clock64(); ++tr_n; } } while (0)
+#define TR_NEXT do { ++tr_tile; } while (0)
+#else
+#define TR_DECL
+#define TR(role, tag) do {} while (0)
+#define TR_NEXT do {} while (0)
+#endif
 
 struct TcArgs {
     CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px]
@@ -198,13 +218,20 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
     const uint32_t tmem = *tptr;
     const uint32_t ws_s = smem_u32(ws_p), hs_s = smem_u32(hs_p), ring_s = smem_u32(ring);
     const uint32_t slots_per_tile = (uint32_t)(KH + NC + 2 * NCH2);
+    const uint32_t ns_magic = 0xffffffffu / NS + 1u;    // seq / NS == umulhi(seq, ns_magic) for seq < 2^29
+    auto slot_of = [&](uint32_t seq, uint32_t& par) -> uint32_t {
+        const uint32_t qd = __umulhi(seq, ns_magic);
+        par = qd & 1u;
+        return seq - qd * NS;
+    };
 
     if (warp == W_TMA) {
         // =========================== TMA producer ===========================
         if (lane == 0) {
             uint32_t seq = 0;
             auto acquire = [&](uint32_t bytes) -> uint32_t {      // next ring slot, armed for `bytes`
-                const uint32_t s = seq % NS, par = (seq / NS) & 1u;
+                uint32_t par;
+                const uint32_t s = slot_of(seq, par);
                 mbar_wait(&bars[B_EMPTY + s], par ^ 1u);
                 mbar_expect_tx(&bars[B_FULL + s], bytes);
                 ++seq;
@@ -249,7 +276,9 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         const int NSC = (NC + 1) / 2;                    // H-phase super-chunks of 32 frames (the last may hold 16)
         constexpr int NSC2 = NCH2 / 2;                   // W-phase super-chunks of 32 pixels
         uint32_t acc_started = 0;
+        TR_DECL
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+            TR(0, 1);
             // ---- H phase ----
             auto issue_S = [&](int j) {                  // S(j): [128 px] x [32 frames], K = comps -> Z[j & 1]
                 if (elect_one()) {
@@ -267,13 +296,16 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 __syncwarp();
             };
             wait(B_HS);
+            TR(0, 2);
             issue_S(0);
             if (NSC > 1) issue_S(1);
+            TR(0, 3);
             for (int j = 0; j < NSC; ++j) {
                 for (int gg = 0; gg < 2; ++gg) {
                     const int c = 2 * j + gg;
                     if (c >= NC) break;
                     wait(B_P0 + gg);
+                    TR(0, 100 + c);
                     if (elect_one()) {
                         const uint32_t z = tmem + T_HZ + 32 * (j & 1) + 16 * gg, e = tmem + T_HE + 32 * gg;
                         const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
@@ -293,6 +325,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             }
             if (elect_one()) mma_commit(&bars[B_ND]);
             __syncwarp();
+            TR(0, 4);
             // ---- W phase ----
             auto issue_S2 = [&](int j) {                 // S'(j)[m]: [128 frames] x [32 px], K = comps -> Z[j & 1][m]
                 if (elect_one()) {
@@ -312,12 +345,15 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 __syncwarp();
             };
             wait(B_HS2);
+            TR(0, 5);
             issue_S2(0);
             issue_S2(1);
+            TR(0, 6);
             for (int j = 0; j < NSC2; ++j) {
                 for (int gg = 0; gg < 2; ++gg) {
                     const int c = 2 * j + gg;
                     wait(B_P20 + gg);
+                    TR(0, 200 + c);
                     if (elect_one()) {
                         const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
                         for (int m = 0; m < MT; ++m) {
@@ -341,6 +377,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             }
             if (elect_one()) mma_commit(&bars[B_AB]);
             __syncwarp();
+            TR(0, 7);
+            TR_NEXT;
         }
     } else {
         // =========================== element-wise warps ===========================
@@ -350,13 +388,15 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         uint32_t ph = 0;
         auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; };
         auto wait_full = [&](uint32_t seq) -> const unsigned char* {
-            const uint32_t s = seq % NS;
-            mbar_wait(&bars[B_FULL + s], (seq / NS) & 1u);
+            uint32_t par;
+            const uint32_t s = slot_of(seq, par);
+            mbar_wait(&bars[B_FULL + s], par);
             return ring + (size_t)s * SLOT;
         };
         auto release = [&](uint32_t seq) {               // this warp is done reading the slot
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[B_EMPTY + seq % NS]);
+            uint32_t par;
+            if (lane == 0) mbar_arrive(&bars[B_EMPTY + slot_of(seq, par)]);
         };
         auto warp_arrive = [&](int bar) {
             __syncwarp();
@@ -366,37 +406,46 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         bool first = true;
         const int NSC = (NC + 1) / 2;
         constexpr int NSC2 = NCH2 / 2;
+        TR_DECL
+#ifdef NMF_TC_TRACE
+        const int tr_role = (q == 0) ? 1 + grp : 0;
+#define TRE(tag) do { if (tr_role) TR(tr_role, tag); } while (0)
+#else
+#define TRE(tag) do {} while (0)
+#endif
 
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
+            TRE(1);
             const long long p = tile * TILE + t;
             const bool p_ok = p < P;
             const long long pc = p_ok ? p : P - 1;
 
-            // ---- H0: this group's 32 components of the H tile: keep h, split into Hs[pixel][comp] ----
-            float h[32];
-            if (grp < KH) {
-                const float* hsl = reinterpret_cast<const float*>(wait_full(sq + grp));
-#pragma unroll
-                for (int j = 0; j < 32; ++j) h[j] = (32 * grp + j < K) ? hsl[j * TILE + t] : 0.f;   // px >= P: zero-filled
-                release(sq + grp);
-            } else {
-#pragma unroll
-                for (int j = 0; j < 32; ++j) h[j] = 0.f;
-            }
+            // ---- H0: this group's 32 components of the H tile are split into Hs[pixel][comp] ----
+            const float* hsl = nullptr;
+            if (grp < KH) hsl = reinterpret_cast<const float*>(wait_full(sq + grp));
+            TRE(2);
             if (!first) { wait(B_AB); }                  // every MMA of the previous tile is complete: Hs is free
             first = false;
+            TRE(3);
 #pragma unroll
             for (int gq = 0; gq < 4; ++gq) {
                 uint32_t p1[4], p2[4], p3[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) split3_pair(h[8 * gq + 2 * j], h[8 * gq + 2 * j + 1], p1[j], p2[j], p3[j]);
+                for (int j = 0; j < 4; ++j) {
+                    const int k0 = 32 * grp + 8 * gq + 2 * j;    // pixels >= P arrive zero-filled
+                    const float h0 = (hsl && k0 < K) ? hsl[(8 * gq + 2 * j) * TILE + t] : 0.f;
+                    const float h1 = (hsl && k0 + 1 < K) ? hsl[(8 * gq + 2 * j + 1) * TILE + t] : 0.f;
+                    split3_pair(h0, h1, p1[j], p2[j], p3[j]);
+                }
                 const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + (4 * grp + gq) * HS_SB;
                 *reinterpret_cast<uint4*>(hs_p + off) = make_uint4(p1[0], p1[1], p1[2], p1[3]);
                 *reinterpret_cast<uint4*>(hs_p + HS_BYTES + off) = make_uint4(p2[0], p2[1], p2[2], p2[3]);
                 *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(p3[0], p3[1], p3[2], p3[3]);
             }
+            if (grp < KH) release(sq + grp);
             fence_proxy_async();
             warp_arrive(B_HS);
+            TRE(4);
 
             // ---- H phase: super-chunk j = chunks 2j (group 0) and 2j + 1 (group 1); thread = (pixel t, 16 frames) ----
             bool pending = false;                        // an ND of this group may still be reading E[grp]
@@ -407,6 +456,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 if (have) {
                     const uint32_t seq = sq + KH + c;
                     const float* xs = reinterpret_cast<const float*>(wait_full(seq));
+                    TRE(190 + j);
                     const int nv = N - FCH * c;          // valid frames of this chunk (>= 16: all)
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
@@ -415,7 +465,9 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     }
                     release(seq);
                 }
+                TRE(100 + j);
                 wait(B_S0 + (j & 1));                    // both groups track every completion of the buffer's barrier
+                TRE(120 + j);
                 if (have) {
                     tc_fence_after();
                     const uint32_t zcol = lane_base + T_HZ + 32 * (j & 1) + 16 * grp;
@@ -423,56 +475,73 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     tmem_ld16(zcol, s);
                     tmem_wait_ld();
                     ew16(x, o, s, zcol, e);
+                    TRE(140 + j);
                     if (pending) { wait(B_NDG0 + grp); tc_fence_after(); }
+                    TRE(160 + j);
                     tmem_st32(lane_base + T_HE + 32 * grp, e);
                     tmem_wait_st();
+                    TRE(170 + j);
                     tc_fence_before();
                     warp_arrive(B_P0 + grp);
+                    TRE(180 + j);
                     pending = true;
                 }
             }
+            TRE(5);
+            // ---- UPD: h' = h * num / max(den, eps); thread = (pixel t, this group's 32 comps) ----
+            // the old h is rebuilt exactly from its three BF16 pieces in Hs (h = h1 + h2 + h3, every partial sum exact)
             if (pending) wait(B_NDG0 + grp);
             wait(B_ND);                                  // Num, Den complete; every stage-1 read of Hs is done
             tc_fence_after();
-
-            // ---- UPD: h' = h * num / max(den, eps); thread = (pixel t, this group's 32 comps) ----
+            TRE(6);
+            {
+                float* hp = H + (size_t)(32 * grp) * P + pc;
 #pragma unroll
-            for (int gq = 0; gq < 4; ++gq) {
-                const int kg = 4 * grp + gq;
-                uint32_t nm[8], dn[8];
-                tmem_ld8(lane_base + T_NUM + 8 * kg, nm);
-                tmem_ld8(lane_base + T_DEN + 8 * kg, dn);
-                tmem_wait_ld();
-                float hn[8];
+                for (int gq = 0; gq < 4; ++gq) {
+                    const int kg = 4 * grp + gq;
+                    const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + kg * HS_SB;
+                    uint32_t nm[8], dn[8];
+                    tmem_ld8(lane_base + T_NUM + 8 * kg, nm);
+                    tmem_ld8(lane_base + T_DEN + 8 * kg, dn);
+                    const uint4 h1 = *reinterpret_cast<const uint4*>(hs_p + off);
+                    const uint4 h2 = *reinterpret_cast<const uint4*>(hs_p + HS_BYTES + off);
+                    const uint4 h3 = *reinterpret_cast<const uint4*>(hs_p + 2 * HS_BYTES + off);
+                    const uint32_t a1[4] = {h1.x, h1.y, h1.z, h1.w}, a2[4] = {h2.x, h2.y, h2.z, h2.w}, a3[4] = {h3.x, h3.y, h3.z, h3.w};
+                    tmem_wait_ld();
+                    float hn[8];
 #pragma unroll
-                for (int j = 0; j < 8; ++j) {
-                    const int k = kg * 8 + j;
-                    float v = 0.f;
-                    if (p_ok && k < K) {
-                        v = (h[8 * gq + j] * __uint_as_float(nm[j])) / fmaxf(__uint_as_float(dn[j]), NMF_EPS);
-                        H[(size_t)k * P + pc] = v;
+                    for (int j = 0; j < 8; ++j, hp += P) {
+                        const int w = j >> 1;
+                        const float hold = (j & 1)
+                            ? (__uint_as_float(a1[w] & 0xffff0000u) + __uint_as_float(a2[w] & 0xffff0000u)) + __uint_as_float(a3[w] & 0xffff0000u)
+                            : (__uint_as_float(a1[w] << 16) + __uint_as_float(a2[w] << 16)) + __uint_as_float(a3[w] << 16);
+                        // padded comps / pixels carry h = 0 and num = 0: v = 0
+                        const float v = __fdividef(hold * __uint_as_float(nm[j]), fmaxf(__uint_as_float(dn[j]), NMF_EPS));
+                        if (p_ok && kg * 8 + j < K) *hp = v;
+                        hn[j] = v;
                     }
-                    hn[j] = v;
-                }
-                uint32_t p1[4], p2[4], p3[4];
+                    uint32_t p1[4], p2[4], p3[4];
 #pragma unroll
-                for (int j = 0; j < 4; ++j) split3_pair(hn[2 * j], hn[2 * j + 1], p1[j], p2[j], p3[j]);
-                const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + kg * HS_SB;
-                *reinterpret_cast<uint4*>(hs_p + off) = make_uint4(p1[0], p1[1], p1[2], p1[3]);
-                *reinterpret_cast<uint4*>(hs_p + HS_BYTES + off) = make_uint4(p2[0], p2[1], p2[2], p2[3]);
-                *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(p3[0], p3[1], p3[2], p3[3]);
+                    for (int j = 0; j < 4; ++j) split3_pair(hn[2 * j], hn[2 * j + 1], p1[j], p2[j], p3[j]);
+                    *reinterpret_cast<uint4*>(hs_p + off) = make_uint4(p1[0], p1[1], p1[2], p1[3]);
+                    *reinterpret_cast<uint4*>(hs_p + HS_BYTES + off) = make_uint4(p2[0], p2[1], p2[2], p2[3]);
+                    *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(p3[0], p3[1], p3[2], p3[3]);
+                }
             }
             fence_proxy_async();
             tc_fence_before();
             warp_arrive(B_HS2);
+            TRE(7);
 
             // ---- W phase: super-chunk j = chunks 2j + grp; thread = (frames t and 128 + t, 16 pixels) ----
             pending = false;
             for (int j = 0; j < NSC2; ++j) {
                 const int c = 2 * j + grp;
                 const uint32_t seq = sq + KH + NC + 2 * c;
+                TRE(200 + j);
                 const unsigned char* xsl = wait_full(seq);
                 const unsigned char* osl = wait_full(seq + 1);
+                TRE(210 + j);
                 for (int m = 0; m < MT; ++m) {
                     const int fr = 128 * m + t;
                     const bool active = 128 * m + 32 * q < N;        // warp-uniform: some lane has a frame
@@ -493,7 +562,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         }
                     }
                     if (m == MT - 1) { release(seq); release(seq + 1); }
-                    if (m == 0) { wait(B_S20 + (j & 1)); tc_fence_after(); }
+                    if (m == 0) { wait(B_S20 + (j & 1)); tc_fence_after(); TRE(220 + j); }
                     uint32_t e[32];
                     if (active) {
                         const uint32_t zcol = lane_base + T_WZ + 32 * (2 * (j & 1) + m) + 16 * grp;
@@ -502,15 +571,20 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         tmem_wait_ld();
                         ew16(x, o, s, zcol, e);
                     }
+                    if (m == 0) TRE(230 + j);
                     if (m == 0 && pending) { wait(B_ABG0 + grp); tc_fence_after(); }
+                    if (m == 0) TRE(240 + j);
                     if (active) tmem_st32(lane_base + T_WE + 32 * (2 * grp + m), e);
                 }
                 tmem_wait_st();
                 tc_fence_before();
                 warp_arrive(B_P20 + grp);
                 pending = true;
+                TRE(250 + j);
             }
             wait(B_ABG0 + grp);
+            TRE(8);
+            TR_NEXT;
         }
         wait(B_AB);                                      // every MMA of the last tile is complete
         tc_fence_after();
@@ -613,6 +687,12 @@ size_t nmf_tc_workspace(const nmf_plan* p) {
 }
 
 bool nmf_tc_available(const nmf_plan* p) { return p->t_ctas != 0; }
+
+#ifdef NMF_TC_TRACE
+extern "C" int nmf_debug_tc_trace(long long* host_out) {
+    return (int)cudaMemcpyFromSymbol(host_out, nmf_tc_trace_buf, sizeof(long long) * 3 * 1024);
+}
+#endif
 
 int nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
     if (!p->t_ctas) return NMF_ERR_UNSUPPORTED;
