@@ -236,20 +236,34 @@ k_w_partial(const float* __restrict__ X, const float* __restrict__ Om, const flo
 // ---------------------------------------------------------------------------
 // Fixed-order reduction of the partial slabs (fp64) + W <- W o A / max(B, eps)
 // ---------------------------------------------------------------------------
-__global__ void k_w_update(const float* __restrict__ slab, float* __restrict__ W, int N, int K,
-                           int KT, int parts) {
+// 256 threads = 8 part lanes x 32 elements: lane q sums the parts q, q + 8, ... in order, the 8 partial sums are
+// then added in lane order -- a fixed association, so the result is bitwise reproducible.
+__global__ void __launch_bounds__(256)
+k_w_update(const float* __restrict__ slab, float* __restrict__ W, int N, int K, int KT, int parts) {
+    __shared__ double sa[8][32], sd[8][32];
     const int b = blockIdx.y;
-    const int i = blockIdx.x * blockDim.x + threadIdx.x;
-    if (i >= N * K) return;
-    const int n = i / K, k = i - n * K;
-    const float* s = slab + (size_t)b * parts * 2 * N * KT + (size_t)n * KT + k;
+    const int e = threadIdx.x & 31, q = threadIdx.x >> 5;
+    const int i = blockIdx.x * 32 + e;
+    const bool ok = i < N * K;
+    const int n = ok ? i / K : 0, k = ok ? i - n * K : 0;
+    const size_t stride = (size_t)2 * N * KT;
+    const float* s = slab + (size_t)b * parts * stride + (size_t)n * KT + k;
     double a = 0.0, d = 0.0;
-    for (int part = 0; part < parts; ++part) {
-        a += (double)s[(size_t)(2 * part) * N * KT];
-        d += (double)s[(size_t)(2 * part + 1) * N * KT];
+    if (ok) {
+#pragma unroll 4
+        for (int part = q; part < parts; part += 8) {
+            a += (double)s[(size_t)part * stride];
+            d += (double)s[(size_t)part * stride + (size_t)N * KT];
+        }
     }
-    float* w = W + (size_t)b * N * K + i;
-    *w = (*w * (float)a) / fmaxf((float)d, NMF_EPS);
+    sa[q][e] = a; sd[q][e] = d;
+    __syncthreads();
+    if (q == 0 && ok) {
+#pragma unroll
+        for (int r = 1; r < 8; ++r) { a += sa[r][e]; d += sd[r][e]; }
+        float* w = W + (size_t)b * N * K + i;
+        *w = (*w * (float)a) / fmaxf((float)d, NMF_EPS);
+    }
 }
 
 // ---- host-side geometry -----------------------------------------------------
@@ -320,8 +334,8 @@ int launch_w(nmf_plan* p, const float* X, const float* Om, float* W, const float
         k_w_partial<KC, W_NF, true><<<grid, threads, smem, p->stream>>>(X, Om, W, H, slab, rows, p->P, p->K, KS, NBc);
     else
         k_w_partial<KC, W_NF, false><<<grid, threads, smem, p->stream>>>(X, Om, W, H, slab, rows, p->P, p->K, KS, NBc);
-    dim3 g2((rows * p->K + 127) / 128, batch);
-    k_w_update<<<g2, 128, 0, p->stream>>>(slab, W, rows, p->K, KC * KS, parts);
+    dim3 g2((rows * p->K + 31) / 32, batch);
+    k_w_update<<<g2, 256, 0, p->stream>>>(slab, W, rows, p->K, KC * KS, parts);
     p->launches += 2;
     return NMF_OK;
 }
@@ -370,8 +384,8 @@ size_t nmf_generic_workspace(const nmf_plan* p) {
 
 int nmf_launch_w_update(nmf_plan* p, const float* slab, float* W, int rows, int K, int KT, int parts,
                         int batch) {
-    dim3 g2((rows * K + 127) / 128, batch);
-    k_w_update<<<g2, 128, 0, p->stream>>>(slab, W, rows, K, KT, parts);
+    dim3 g2((rows * K + 31) / 32, batch);
+    k_w_update<<<g2, 256, 0, p->stream>>>(slab, W, rows, K, KT, parts);
     p->launches++;
     return NMF_OK;
 }

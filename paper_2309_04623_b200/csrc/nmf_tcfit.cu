@@ -154,7 +154,7 @@ struct TcArgs {
 };
 
 // mbarrier slots
-enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P0, B_P1, B_NDG0, B_NDG1, B_ND, B_S20, B_S21, B_P20, B_P21, B_ABG0, B_ABG1, B_AB,
+enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P0, B_P1, B_NDG0, B_NDG1, B_ND, B_S2, B_S2_LAST = B_S2 + 3, B_P20, B_P21, B_ABG0, B_ABG1, B_AB,
        B_FULL, B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
 
 template <int KS>
@@ -185,7 +185,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1);
         mbar_init(&bars[B_P0], 4); mbar_init(&bars[B_P1], 4); mbar_init(&bars[B_ND], 1);
         mbar_init(&bars[B_NDG0], 1); mbar_init(&bars[B_NDG1], 1);
-        mbar_init(&bars[B_S20], 1); mbar_init(&bars[B_S21], 1);
+        for (int i = 0; i < 4; ++i) mbar_init(&bars[B_S2 + i], 1);     // S'[jb][m] ready
         mbar_init(&bars[B_P20], 4); mbar_init(&bars[B_P21], 4); mbar_init(&bars[B_AB], 1);
         mbar_init(&bars[B_ABG0], 1); mbar_init(&bars[B_ABG1], 1);
         for (uint32_t s = 0; s < NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 4); }
@@ -339,8 +339,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                             for (int ks = 0; ks < KS; ++ks)
                                 mma16_ss(d, d_ws_k[pa[pr]] + aoff + ks * ws_kstep, d_hs_k[pb[pr]] + boff + ks * hs_kstep,
                                          id_s32, (pr | ks) ? 1u : 0u);
+                        mma_commit(&bars[B_S2 + 2 * (j & 1) + m]);
                     }
-                    mma_commit(&bars[B_S20 + (j & 1)]);
                 }
                 __syncwarp();
             };
@@ -424,23 +424,23 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             const float* hsl = nullptr;
             if (grp < KH) hsl = reinterpret_cast<const float*>(wait_full(sq + grp));
             TRE(2);
+            uint32_t hp1[16], hp2[16], hp3[16];
+#pragma unroll
+            for (int j = 0; j < 16; ++j) {
+                const int k0 = 32 * grp + 2 * j;         // pixels >= P arrive zero-filled
+                const float h0 = (hsl && k0 < K) ? hsl[(2 * j) * TILE + t] : 0.f;
+                const float h1 = (hsl && k0 + 1 < K) ? hsl[(2 * j + 1) * TILE + t] : 0.f;
+                split3_pair(h0, h1, hp1[j], hp2[j], hp3[j]);
+            }
             if (!first) { wait(B_AB); }                  // every MMA of the previous tile is complete: Hs is free
             first = false;
             TRE(3);
 #pragma unroll
             for (int gq = 0; gq < 4; ++gq) {
-                uint32_t p1[4], p2[4], p3[4];
-#pragma unroll
-                for (int j = 0; j < 4; ++j) {
-                    const int k0 = 32 * grp + 8 * gq + 2 * j;    // pixels >= P arrive zero-filled
-                    const float h0 = (hsl && k0 < K) ? hsl[(8 * gq + 2 * j) * TILE + t] : 0.f;
-                    const float h1 = (hsl && k0 + 1 < K) ? hsl[(8 * gq + 2 * j + 1) * TILE + t] : 0.f;
-                    split3_pair(h0, h1, p1[j], p2[j], p3[j]);
-                }
                 const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + (4 * grp + gq) * HS_SB;
-                *reinterpret_cast<uint4*>(hs_p + off) = make_uint4(p1[0], p1[1], p1[2], p1[3]);
-                *reinterpret_cast<uint4*>(hs_p + HS_BYTES + off) = make_uint4(p2[0], p2[1], p2[2], p2[3]);
-                *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(p3[0], p3[1], p3[2], p3[3]);
+                *reinterpret_cast<uint4*>(hs_p + off) = make_uint4(hp1[4 * gq], hp1[4 * gq + 1], hp1[4 * gq + 2], hp1[4 * gq + 3]);
+                *reinterpret_cast<uint4*>(hs_p + HS_BYTES + off) = make_uint4(hp2[4 * gq], hp2[4 * gq + 1], hp2[4 * gq + 2], hp2[4 * gq + 3]);
+                *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(hp3[4 * gq], hp3[4 * gq + 1], hp3[4 * gq + 2], hp3[4 * gq + 3]);
             }
             if (grp < KH) release(sq + grp);
             fence_proxy_async();
@@ -562,7 +562,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         }
                     }
                     if (m == MT - 1) { release(seq); release(seq + 1); }
-                    if (m == 0) { wait(B_S20 + (j & 1)); tc_fence_after(); TRE(220 + j); }
+                    wait(B_S2 + 2 * (j & 1) + m); tc_fence_after();
+                    if (m == 0) TRE(220 + j);
                     uint32_t e[32];
                     if (active) {
                         const uint32_t zcol = lane_base + T_WZ + 32 * (2 * (j & 1) + m) + 16 * grp;
