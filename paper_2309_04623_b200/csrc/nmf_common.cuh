@@ -80,6 +80,8 @@ size_t nmf_tc_workspace(const nmf_plan* p);
 bool   nmf_tc_available(const nmf_plan* p);
 int    nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
                   int iters, int batch);
+int    nmf_tc_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C,
+                      int M, int iters);
 // auxiliaries
 size_t nmf_aux_workspace(const nmf_plan* p);
 int    nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C,

@@ -151,6 +151,7 @@ struct TcArgs {
     int MT;                    // 128-frame M tiles of the W phase (1 or 2)
     int KH;                    // 32-component slots of the H tile (1 or 2)
     int NS;                    // ring slots
+    int proj;                  // 1: projection (a9): H is fixed, only the W phase runs (X = targets, Om = omega, W = coef)
 };
 
 // mbarrier slots
@@ -217,7 +218,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
     tc_fence_after();
     const uint32_t tmem = *tptr;
     const uint32_t ws_s = smem_u32(ws_p), hs_s = smem_u32(hs_p), ring_s = smem_u32(ring);
-    const uint32_t slots_per_tile = (uint32_t)(KH + NC + 2 * NCH2);
+    const bool proj = g.proj != 0;
+    const uint32_t slots_per_tile = (uint32_t)(KH + (proj ? 0 : NC) + 2 * NCH2);
     const uint32_t ns_magic = 0xffffffffu / NS + 1u;    // seq / NS == umulhi(seq, ns_magic) for seq < 2^29
     auto slot_of = [&](uint32_t seq, uint32_t& par) -> uint32_t {
         const uint32_t qd = __umulhi(seq, ns_magic);
@@ -243,7 +245,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     const uint32_t s = acquire(32 * TILE * 4);
                     tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
                 }
-                for (int c = 0; c < NC; ++c) {
+                for (int c = 0; c < (proj ? 0 : NC); ++c) {
                     const uint32_t s = acquire(2 * FCH * TILE * 4);
                     tma_load_2d(ring_s + s * SLOT, &g.mXh, p0, b * N + FCH * c, &bars[B_FULL + s]);
                     tma_load_2d(ring_s + s * SLOT + FCH * TILE * 4, &g.mOh, p0, b * N + FCH * c, &bars[B_FULL + s]);
@@ -297,6 +299,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             };
             wait(B_HS);
             TR(0, 2);
+            if (!proj) {
             issue_S(0);
             if (NSC > 1) issue_S(1);
             TR(0, 3);
@@ -326,6 +329,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             if (elect_one()) mma_commit(&bars[B_ND]);
             __syncwarp();
             TR(0, 4);
+            }
             // ---- W phase ----
             auto issue_S2 = [&](int j) {                 // S'(j)[m]: [128 frames] x [32 px], K = comps -> Z[j & 1][m]
                 if (elect_one()) {
@@ -344,7 +348,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 }
                 __syncwarp();
             };
-            wait(B_HS2);
+            if (!proj) wait(B_HS2);
             TR(0, 5);
             issue_S2(0);
             issue_S2(1);
@@ -447,8 +451,9 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             warp_arrive(B_HS);
             TRE(4);
 
+            bool pending = false;                        // an ND / AB of this group may still be reading E[grp]
+            if (!proj) {
             // ---- H phase: super-chunk j = chunks 2j (group 0) and 2j + 1 (group 1); thread = (pixel t, 16 frames) ----
-            bool pending = false;                        // an ND of this group may still be reading E[grp]
             for (int j = 0; j < NSC; ++j) {
                 const int c = 2 * j + grp;
                 const bool have = c < NC;
@@ -463,7 +468,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         x[i] = xs[i * TILE + t];
                         o[i] = i < nv ? xs[FCH * TILE + i * TILE + t] : 0.f;
                     }
-                    release(seq);
                 }
                 TRE(100 + j);
                 wait(B_S0 + (j & 1));                    // both groups track every completion of the buffer's barrier
@@ -475,6 +479,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     tmem_ld16(zcol, s);
                     tmem_wait_ld();
                     ew16(x, o, s, zcol, e);
+                    release(sq + KH + c);                // only now: every x, o value has been consumed (a release right
+                                                         // after issuing the loads raced with the refill of the slot)
                     TRE(140 + j);
                     if (pending) { wait(B_NDG0 + grp); tc_fence_after(); }
                     TRE(160 + j);
@@ -532,12 +538,13 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             tc_fence_before();
             warp_arrive(B_HS2);
             TRE(7);
+            }   // !proj
 
             // ---- W phase: super-chunk j = chunks 2j + grp; thread = (frames t and 128 + t, 16 pixels) ----
             pending = false;
             for (int j = 0; j < NSC2; ++j) {
                 const int c = 2 * j + grp;
-                const uint32_t seq = sq + KH + NC + 2 * c;
+                const uint32_t seq = sq + KH + (proj ? 0 : NC) + 2 * c;
                 TRE(200 + j);
                 const unsigned char* xsl = wait_full(seq);
                 const unsigned char* osl = wait_full(seq + 1);
@@ -561,7 +568,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                             for (int i = 0; i < 16; ++i) { x[i] = 0.f; o[i] = 0.f; }
                         }
                     }
-                    if (m == MT - 1) { release(seq); release(seq + 1); }
                     wait(B_S2 + 2 * (j & 1) + m); tc_fence_after();
                     if (m == 0) TRE(220 + j);
                     uint32_t e[32];
@@ -577,6 +583,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     if (m == 0) TRE(240 + j);
                     if (active) tmem_st32(lane_base + T_WE + 32 * (2 * grp + m), e);
                 }
+                release(seq); release(seq + 1);          // after the values were consumed (see the H phase)
                 tmem_wait_st();
                 tc_fence_before();
                 warp_arrive(B_P20 + grp);
@@ -684,7 +691,10 @@ void nmf_tc_configure(nmf_plan* p) {
 
 size_t nmf_tc_workspace(const nmf_plan* p) {
     if (!p->t_ctas) return 0;
-    return (size_t)p->batch * p->t_ctas * 2 * p->N * KP * sizeof(float);
+    const int prow = p->max_targets < 256 ? p->max_targets : 256;             // projection: <= 256 frames per pass
+    const size_t fit = (size_t)p->batch * p->t_ctas * 2 * p->N * KP * sizeof(float);
+    const size_t proj = (size_t)p->t_ctas * 2 * prow * KP * sizeof(float);
+    return fit > proj ? fit : proj;
 }
 
 bool nmf_tc_available(const nmf_plan* p) { return p->t_ctas != 0; }
@@ -695,20 +705,23 @@ extern "C" int nmf_debug_tc_trace(long long* host_out) {
 }
 #endif
 
-int nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
-    if (!p->t_ctas) return NMF_ERR_UNSUPPORTED;
+namespace {
+// one launch sequence: `iters` x { fused tile kernel ; fixed-order reduce + update of W (or coef) }
+int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* H, int rows, int iters, int batch, bool proj) {
     TcArgs a;
-    const long long rows = (long long)batch * p->N;
+    const long long trows = (long long)batch * rows;
     if (!make_map(&a.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) ||
-        !make_map(&a.mXh, X, rows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om, rows, p->P, FCH, TILE, false) ||
-        !make_map(&a.mXw, X, rows, p->P, p->N, PCH, true) || !make_map(&a.mOw, Om, rows, p->P, p->N, PCH, true)) {
+        !make_map(&a.mXh, X, trows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om, trows, p->P, FCH, TILE, false) ||
+        !make_map(&a.mXw, X, trows, p->P, rows, PCH, true) || !make_map(&a.mOw, Om, trows, p->P, rows, PCH, true)) {
         if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
         return NMF_ERR_CUDA;
     }
-    a.W = W; a.H = H; a.slab = reinterpret_cast<float*>(p->ws);
-    a.N = p->N; a.K = p->K; a.P = p->P; a.n_tiles = (p->P + TILE - 1) / TILE;
-    a.NF = (p->N + FCH - 1) / FCH * FCH; a.NC = a.NF / FCH; a.MT = (p->N + 127) / 128;
-    a.KH = (p->K + 31) / 32; a.NS = p->t_nst;
+    a.W = W; a.H = const_cast<float*>(H); a.slab = reinterpret_cast<float*>(p->ws);
+    a.N = rows; a.K = p->K; a.P = p->P; a.n_tiles = (p->P + TILE - 1) / TILE;
+    a.NF = (rows + FCH - 1) / FCH * FCH; a.NC = a.NF / FCH; a.MT = (rows + 127) / 128;
+    a.KH = (p->K + 31) / 32; a.proj = proj ? 1 : 0;
+    long long ns = ((long long)SMEM_MAX - (long long)tc_smem_fixed(a.NF)) / SLOT;
+    a.NS = (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
     const int KS = (p->K + 15) / 16;
     const size_t smem = tc_smem_fixed(a.NF) + (size_t)a.NS * SLOT;
     const dim3 grid(p->t_ctas, batch);
@@ -722,9 +735,27 @@ int nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
         }
         NMF_CUDA_TRY(p, e);
         p->launches++;
-        int rc = nmf_launch_w_update(p, a.slab, W, p->N, p->K, KP, p->t_ctas, batch);
+        int rc = nmf_launch_w_update(p, a.slab, W, rows, p->K, KP, p->t_ctas, batch);
         if (rc) return rc;
     }
     NMF_CUDA_TRY(p, cudaGetLastError());
+    return NMF_OK;
+}
+}  // namespace
+
+int nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
+    if (!p->t_ctas) return NMF_ERR_UNSUPPORTED;
+    return tc_run(p, X, Om, W, H, p->N, iters, batch, false);
+}
+
+// Projection (a9) on the tensor cores: the W phase alone with H fixed, X = targets, Omega = omega, W = coef.
+// Frames are handled 256 at a time (the W phase holds two 128-row M tiles).
+int nmf_tc_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C, int M, int iters) {
+    if (!p->t_ctas || !om) return NMF_ERR_UNSUPPORTED;
+    for (int m0 = 0; m0 < M; m0 += 256) {
+        const int rows = M - m0 < 256 ? M - m0 : 256;
+        int rc = tc_run(p, T + (size_t)m0 * p->P, om + (size_t)m0 * p->P, C + (size_t)m0 * p->K, H, rows, iters, 1, true);
+        if (rc) return rc;
+    }
     return NMF_OK;
 }
