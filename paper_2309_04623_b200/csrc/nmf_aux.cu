@@ -5,39 +5,62 @@
 namespace {
 
 constexpr int SUB_MC = 32;      // science frames per pass (accumulators per thread)
-constexpr int SUB_THREADS = 256;
+constexpr int SUB_THREADS = 128;
+constexpr int SUB_PX = 4;       // pixels per thread (one 128-bit column segment of H, T, omega, out)
 constexpr int OBJ_THREADS = 128;
 
 // out[m,p] = t[m,p] - f[m] * sum_k c[m,k] H[k,p]; `fill` where omega[m,p] == 0.
-// One pixel per thread, up to SUB_MC frames at once so H is streamed once per pass.
-__global__ void __launch_bounds__(SUB_THREADS)
+// Four pixels per thread and up to SUB_MC frames at once: H is streamed once per pass with 128-bit loads, the
+// coefficients come as 128-bit shared-memory broadcasts (cs[k][m], four frames per load), 128 FFMA per k.
+__global__ void __launch_bounds__(SUB_THREADS, 3)
 k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float* __restrict__ C,
            const float* __restrict__ om, const float* __restrict__ factor, float fill,
            float* __restrict__ out, int M, long long P, int K, int m0) {
-    extern __shared__ float cs[];   // [SUB_MC][K]
+    extern __shared__ __align__(16) float cs[];   // [K][SUB_MC]
     const int mc = min(SUB_MC, M - m0);
     for (int i = threadIdx.x; i < SUB_MC * K; i += SUB_THREADS) {
-        int m = i / K, k = i - m * K;
+        const int k = i / SUB_MC, m = i - k * SUB_MC;
         cs[i] = m < mc ? C[(size_t)(m0 + m) * K + k] : 0.f;
     }
     __syncthreads();
-    const long long p = (long long)blockIdx.x * SUB_THREADS + threadIdx.x;
-    if (p >= P) return;
-    float acc[SUB_MC];
+    const long long p = ((long long)blockIdx.x * SUB_THREADS + threadIdx.x) * SUB_PX;
+    if (p >= P) return;                            // P % 4 == 0: a segment is all in or all out
+    float acc[SUB_MC][SUB_PX];
 #pragma unroll
-    for (int m = 0; m < SUB_MC; ++m) acc[m] = 0.f;
-    for (int k = 0; k < K; ++k) {
-        const float h = __ldg(H + (size_t)k * P + p);
+    for (int m = 0; m < SUB_MC; ++m)
 #pragma unroll
-        for (int m = 0; m < SUB_MC; ++m) acc[m] = fmaf(cs[m * K + k], h, acc[m]);
+        for (int q = 0; q < SUB_PX; ++q) acc[m][q] = 0.f;
+    const float* hp = H + p;
+#pragma unroll 2
+    for (int k = 0; k < K; ++k, hp += P) {
+        const float4 h = __ldg(reinterpret_cast<const float4*>(hp));
+#pragma unroll
+        for (int m4 = 0; m4 < SUB_MC / 4; ++m4) {
+            const float4 c = *reinterpret_cast<const float4*>(cs + k * SUB_MC + 4 * m4);
+            const float cc[4] = {c.x, c.y, c.z, c.w};
+#pragma unroll
+            for (int u = 0; u < 4; ++u) {
+                acc[4 * m4 + u][0] = fmaf(cc[u], h.x, acc[4 * m4 + u][0]);
+                acc[4 * m4 + u][1] = fmaf(cc[u], h.y, acc[4 * m4 + u][1]);
+                acc[4 * m4 + u][2] = fmaf(cc[u], h.z, acc[4 * m4 + u][2]);
+                acc[4 * m4 + u][3] = fmaf(cc[u], h.w, acc[4 * m4 + u][3]);
+            }
+        }
     }
 #pragma unroll
     for (int m = 0; m < SUB_MC; ++m) {
         if (m < mc) {
             const size_t i = (size_t)(m0 + m) * P + p;
-            const bool live = om ? (om[i] > 0.f) : true;
             const float f = factor ? factor[m0 + m] : 1.f;
-            out[i] = live ? (T[i] - f * acc[m]) : fill;
+            const float4 t = __ldg(reinterpret_cast<const float4*>(T + i));
+            float4 o = make_float4(1.f, 1.f, 1.f, 1.f);
+            if (om) o = __ldg(reinterpret_cast<const float4*>(om + i));
+            float4 r;                              // omega == 0: T may hold NaN/Inf there (G5) -> select
+            r.x = o.x > 0.f ? t.x - f * acc[m][0] : fill;
+            r.y = o.y > 0.f ? t.y - f * acc[m][1] : fill;
+            r.z = o.z > 0.f ? t.z - f * acc[m][2] : fill;
+            r.w = o.w > 0.f ? t.w - f * acc[m][3] : fill;
+            *reinterpret_cast<float4*>(out + i) = r;
         }
     }
 }
@@ -84,7 +107,8 @@ size_t nmf_aux_workspace(const nmf_plan* p) {
 
 int nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C, const float* om,
                      const float* factor, float fill, float* out, int M) {
-    const unsigned grid = (unsigned)((p->P + SUB_THREADS - 1) / SUB_THREADS);
+    const long long per_cta = (long long)SUB_THREADS * SUB_PX;
+    const unsigned grid = (unsigned)((p->P + per_cta - 1) / per_cta);
     const size_t smem = sizeof(float) * SUB_MC * p->K;
     for (int m0 = 0; m0 < M; m0 += SUB_MC) {
         k_subtract<<<grid, SUB_THREADS, smem, p->stream>>>(H, T, C, om, factor, fill, out, M, p->P, p->K, m0);
