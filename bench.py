@@ -147,7 +147,7 @@ def run_reference(args, rank):
 def run_ours(args, rank, world, local_rank):
     import torch
     import torch.distributed as dist
-    from paper_2309_04623_b200 import inputs, nmf
+    from paper_2309_04623_b200 import inputs, nmf, sharding
 
     if not torch.cuda.is_available():
         raise SystemExit("bench.py: no CUDA device (the product has no CPU fallback)")
@@ -156,7 +156,7 @@ def run_ours(args, rank, world, local_rank):
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
     wl = WORKLOADS[args.workload]
     # every rank fits its own replica (per-rank seed): independent problems, no collective
-    p = inputs.make_stis(N=wl["N"], S=wl["S"], K=wl["K"], M=wl["M"], seed=3003 + 7919 * rank)
+    p = inputs.make_stis(N=wl["N"], S=wl["S"], K=wl["K"], M=wl["M"], seed=sharding.replica_seed(3003, rank))
     N, P, K, M = p.N, p.P, p.K, p.M
     plan = nmf.Plan(N, P, K, max_targets=M, variant=args.variant)
     pin = lambda a: torch.from_numpy(a).pin_memory()
@@ -196,10 +196,7 @@ def run_ours(args, rank, world, local_rank):
     launches = plan.launch_count - l0
     ms_total = e0.elapsed_time(e1)
     fit_ms = [a.elapsed_time(b) for a, b in fit_ev]
-    t = torch.tensor([ms_total], device="cuda")
-    if world > 1:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_max = float(t.item())
+    ms_max = sharding.max_over_ranks(ms_total, "cuda")
     assert torch.isfinite(W).all() and torch.isfinite(H).all()
 
     # ---- end-to-end through the C-ABI with host buffers (copies inside the timed region) ----
@@ -222,10 +219,7 @@ def run_ours(args, rank, world, local_rank):
     e2e_call()
     torch.cuda.synchronize()
     e2e_s = time.perf_counter() - t0
-    te = torch.tensor([e2e_s], device="cuda")
-    if world > 1:
-        dist.all_reduce(te, op=dist.ReduceOp.MAX)
-    e2e_s = float(te.item())
+    e2e_s = sharding.max_over_ranks(e2e_s, "cuda")
     h2d = 4.0 * (2 * N * P + N * K + K * P) + 4.0 * (K * P + 2 * M * P + M * K)
     d2h = 4.0 * (N * K + K * P) + 4.0 * (M * K + M * P)
 
