@@ -31,19 +31,29 @@ k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float
 #pragma unroll
         for (int q = 0; q < SUB_PX; ++q) acc[m][q] = 0.f;
     const float* hp = H + p;
-#pragma unroll 2
-    for (int k = 0; k < K; ++k, hp += P) {
-        const float4 h = __ldg(reinterpret_cast<const float4*>(hp));
+    constexpr int KU = 5;                          // H rows in flight per thread (128-bit loads)
+    for (int k0 = 0; k0 < K; k0 += KU) {
+        float4 hv[KU];
 #pragma unroll
-        for (int m4 = 0; m4 < SUB_MC / 4; ++m4) {
-            const float4 c = *reinterpret_cast<const float4*>(cs + k * SUB_MC + 4 * m4);
-            const float cc[4] = {c.x, c.y, c.z, c.w};
+        for (int u = 0; u < KU; ++u)
+            hv[u] = (k0 + u < K) ? __ldg(reinterpret_cast<const float4*>(hp + (size_t)(k0 + u) * P)) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-            for (int u = 0; u < 4; ++u) {
-                acc[4 * m4 + u][0] = fmaf(cc[u], h.x, acc[4 * m4 + u][0]);
-                acc[4 * m4 + u][1] = fmaf(cc[u], h.y, acc[4 * m4 + u][1]);
-                acc[4 * m4 + u][2] = fmaf(cc[u], h.z, acc[4 * m4 + u][2]);
-                acc[4 * m4 + u][3] = fmaf(cc[u], h.w, acc[4 * m4 + u][3]);
+        for (int u = 0; u < KU; ++u) {
+            if (k0 + u < K) {
+                const float4 h = hv[u];
+                const float* ck = cs + (k0 + u) * SUB_MC;
+#pragma unroll
+                for (int m4 = 0; m4 < SUB_MC / 4; ++m4) {
+                    const float4 c = *reinterpret_cast<const float4*>(ck + 4 * m4);
+                    const float cc[4] = {c.x, c.y, c.z, c.w};
+#pragma unroll
+                    for (int v = 0; v < 4; ++v) {
+                        acc[4 * m4 + v][0] = fmaf(cc[v], h.x, acc[4 * m4 + v][0]);
+                        acc[4 * m4 + v][1] = fmaf(cc[v], h.y, acc[4 * m4 + v][1]);
+                        acc[4 * m4 + v][2] = fmaf(cc[v], h.z, acc[4 * m4 + v][2]);
+                        acc[4 * m4 + v][3] = fmaf(cc[v], h.w, acc[4 * m4 + v][3]);
+                    }
+                }
             }
         }
     }
