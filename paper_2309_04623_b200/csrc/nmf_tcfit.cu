@@ -54,8 +54,10 @@ constexpr uint32_t T_NUM = 0, T_DEN = 64;  // H phase: Num^T, Den^T [pixel][64]
 constexpr uint32_t T_HZ = 128;             //   Z[jb] at T_HZ + 32 jb: S of super-chunk j (jb = j & 1); group g owns columns
                                            //   16 g .. 16 g + 15 and overwrites them in place with R1 (8) and R2 (8)
 constexpr uint32_t T_HE = 192;             //   E[g] at T_HE + 32 g: R3, Q1, Q2, Q3 (8 columns each), single-buffered
-constexpr uint32_t T_WZ = 0;               // W phase: Z[jb][m] at 32 (2 jb + m)   (Num/Den are dead by then)
-constexpr uint32_t T_WE = 128;             //   E[g][m] at T_WE + 32 (2 g + m)
+constexpr uint32_t T_WZ = 0;               // W phase, one 128-frame M tile at a time: Z[jb] at 32 jb (Num/Den are dead by then)
+constexpr uint32_t T_WE = 64;              //   E[g] at T_WE + 32 g
+constexpr uint32_t T_WT = 128;             //   the M tile's rows of W as TMEM A operand: piece i at T_WT + 32 i (comps 2c, 2c+1
+                                           //   in column c), so the S' MMAs read A from TMEM and run at the tensor rate
 constexpr uint32_t T_ACC = 256;            // A_acc[m] at T_ACC + 128 m, B_acc[m] at + 64 (persistent over tiles)
 constexpr uint32_t O_R3 = 0, O_Q1 = 8, O_Q2 = 16, O_Q3 = 24;   // inside an E buffer
 
@@ -143,7 +145,7 @@ __device__ long long nmf_tc_trace_buf[3][1024];
 struct TcArgs {
     CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px]
     CUtensorMap mXh, mOh;      // X, Om [B*N, P] box [16 frames][128 px]          (H phase)
-    CUtensorMap mXw, mOw;      // X, Om [B*N, P] box [N frames][16 px], 64-byte swizzle (W phase)
+    CUtensorMap mXw, mOw;      // X, Om [B*N, P] box [128 frames][16 px], 64-byte swizzle (W phase, one M tile)
     const float* W; float* H; float* slab;
     int N, K; long long P; long long n_tiles;
     int NF;                    // frames padded to a multiple of 16 (rows of the W pieces)
@@ -155,7 +157,7 @@ struct TcArgs {
 };
 
 // mbarrier slots
-enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P0, B_P1, B_NDG0, B_NDG1, B_ND, B_S2, B_S2_LAST = B_S2 + 3, B_P20, B_P21, B_ABG0, B_ABG1, B_AB,
+enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P0, B_P1, B_NDG0, B_NDG1, B_ND, B_S20, B_S21, B_P20, B_P21, B_ABG0, B_ABG1, B_AB, B_WT,
        B_FULL, B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
 
 template <int KS>
@@ -186,7 +188,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1);
         mbar_init(&bars[B_P0], 4); mbar_init(&bars[B_P1], 4); mbar_init(&bars[B_ND], 1);
         mbar_init(&bars[B_NDG0], 1); mbar_init(&bars[B_NDG1], 1);
-        for (int i = 0; i < 4; ++i) mbar_init(&bars[B_S2 + i], 1);     // S'[jb][m] ready
+        mbar_init(&bars[B_S20], 1); mbar_init(&bars[B_S21], 1); mbar_init(&bars[B_WT], EW_WARPS);
         mbar_init(&bars[B_P20], 4); mbar_init(&bars[B_P21], 4); mbar_init(&bars[B_AB], 1);
         mbar_init(&bars[B_ABG0], 1); mbar_init(&bars[B_ABG1], 1);
         for (uint32_t s = 0; s < NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 4); }
@@ -219,7 +221,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
     const uint32_t tmem = *tptr;
     const uint32_t ws_s = smem_u32(ws_p), hs_s = smem_u32(hs_p), ring_s = smem_u32(ring);
     const bool proj = g.proj != 0;
-    const uint32_t slots_per_tile = (uint32_t)(KH + (proj ? 0 : NC) + 2 * NCH2);
+    const int NCR = proj ? 0 : NC;                       // H-phase chunks (none in projection mode)
+    const uint32_t slots_per_tile = (uint32_t)(KH + NCR + MT * NCH2);
     const uint32_t ns_magic = 0xffffffffu / NS + 1u;    // seq / NS == umulhi(seq, ns_magic) for seq < 2^29
     auto slot_of = [&](uint32_t seq, uint32_t& par) -> uint32_t {
         const uint32_t qd = __umulhi(seq, ns_magic);
@@ -245,17 +248,17 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     const uint32_t s = acquire(32 * TILE * 4);
                     tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
                 }
-                for (int c = 0; c < (proj ? 0 : NC); ++c) {
+                for (int c = 0; c < NCR; ++c) {
                     const uint32_t s = acquire(2 * FCH * TILE * 4);
                     tma_load_2d(ring_s + s * SLOT, &g.mXh, p0, b * N + FCH * c, &bars[B_FULL + s]);
                     tma_load_2d(ring_s + s * SLOT + FCH * TILE * 4, &g.mOh, p0, b * N + FCH * c, &bars[B_FULL + s]);
                 }
-                for (int c = 0; c < NCH2; ++c) {
-                    uint32_t s = acquire((uint32_t)N * PCH * 4);
-                    tma_load_2d(ring_s + s * SLOT, &g.mXw, p0 + PCH * c, b * N, &bars[B_FULL + s]);
-                    s = acquire((uint32_t)N * PCH * 4);
-                    tma_load_2d(ring_s + s * SLOT, &g.mOw, p0 + PCH * c, b * N, &bars[B_FULL + s]);
-                }
+                for (int m = 0; m < MT; ++m)             // W phase: M tile m's 128 rows of X and Omega, 16 px at a time
+                    for (int c = 0; c < NCH2; ++c) {
+                        const uint32_t s = acquire(2 * 128 * PCH * 4);
+                        tma_load_2d(ring_s + s * SLOT, &g.mXw, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
+                        tma_load_2d(ring_s + s * SLOT + 128 * PCH * 4, &g.mOw, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
+                    }
             }
         }
     } else if (warp == W_MMA) {
@@ -330,54 +333,52 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             __syncwarp();
             TR(0, 4);
             }
-            // ---- W phase ----
-            auto issue_S2 = [&](int j) {                 // S'(j)[m]: [128 frames] x [32 px], K = comps -> Z[j & 1][m]
+            // ---- W phase: one 128-frame M tile at a time; A of S' = the tile's rows of W, staged in TMEM ----
+            auto issue_S2 = [&](int j) {                 // S'(j): [128 frames] x [32 px], K = comps -> Z[j & 1]
                 if (elect_one()) {
                     const uint32_t boff = (uint32_t)(j * 4 * 128) >> 4;
-                    for (int m = 0; m < MT; ++m) {
-                        const uint32_t d = tmem + T_WZ + 32 * (2 * (j & 1) + m);
-                        const uint32_t aoff = (uint32_t)(m * 16 * 128) >> 4;
+                    const uint32_t d = tmem + T_WZ + 32 * (j & 1);
 #pragma unroll
-                        for (int pr = 0; pr < 6; ++pr)
+                    for (int pr = 0; pr < 6; ++pr)
 #pragma unroll
-                            for (int ks = 0; ks < KS; ++ks)
-                                mma16_ss(d, d_ws_k[pa[pr]] + aoff + ks * ws_kstep, d_hs_k[pb[pr]] + boff + ks * hs_kstep,
-                                         id_s32, (pr | ks) ? 1u : 0u);
-                        mma_commit(&bars[B_S2 + 2 * (j & 1) + m]);
-                    }
+                        for (int ks = 0; ks < KS; ++ks)
+                            mma16_ts(d, tmem + T_WT + 32 * pa[pr] + 8 * ks, d_hs_k[pb[pr]] + boff + ks * hs_kstep,
+                                     id_s32, (pr | ks) ? 1u : 0u);
+                    mma_commit(&bars[B_S20 + (j & 1)]);
                 }
                 __syncwarp();
             };
-            if (!proj) wait(B_HS2);
+            if (!proj) wait(B_HS2);                      // H' pieces in Hs and W tile 0 in TMEM are in place
             TR(0, 5);
-            issue_S2(0);
-            issue_S2(1);
-            TR(0, 6);
-            for (int j = 0; j < NSC2; ++j) {
-                for (int gg = 0; gg < 2; ++gg) {
-                    const int c = 2 * j + gg;
-                    wait(B_P20 + gg);
-                    TR(0, 200 + c);
-                    if (elect_one()) {
-                        const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
-                        for (int m = 0; m < MT; ++m) {
-                            const uint32_t z = tmem + T_WZ + 32 * (2 * (j & 1) + m) + 16 * gg;
-                            const uint32_t e = tmem + T_WE + 32 * (2 * gg + m);
+            for (int m = 0; m < MT; ++m) {
+                if (m > 0) wait(B_WT);                   // W tile m staged (every S' of tile m - 1 has completed)
+                issue_S2(0);
+                issue_S2(1);
+                TR(0, 6);
+                for (int j = 0; j < NSC2; ++j) {
+                    for (int gg = 0; gg < 2; ++gg) {
+                        const int c = 2 * j + gg;
+                        wait(B_P20 + gg);
+                        TR(0, 200 + 10 * m + c);
+                        if (elect_one()) {
+                            const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
+                            const uint32_t z = tmem + T_WZ + 32 * (j & 1) + 16 * gg;
+                            const uint32_t e = tmem + T_WE + 32 * gg;
                             const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
                             const uint32_t a_r[3] = {z, z + 8, e + O_R3};
 #pragma unroll
                             for (int pr = 0; pr < 6; ++pr) {
-                                const uint32_t acc = (acc_started || pr > 0) ? 1u : 0u;
+                                const uint32_t acc = (((acc_started >> m) & 1u) || pr > 0) ? 1u : 0u;
                                 mma16_ts(tmem + T_ACC + 128 * m, a_q[pa[pr]], d_hs_mn[pb[pr]] + boff, id_nd, acc);
                                 mma16_ts(tmem + T_ACC + 128 * m + 64, a_r[pa[pr]], d_hs_mn[pb[pr]] + boff, id_nd, acc);
                             }
+                            mma_commit(&bars[B_ABG0 + gg]);
                         }
-                        mma_commit(&bars[B_ABG0 + gg]);
+                        __syncwarp();
+                        acc_started |= 1u << m;
                     }
-                    __syncwarp();
-                    acc_started = 1;
+                    if (j + 2 < NSC2) issue_S2(j + 2);
                 }
-                if (j + 2 < NSC2) issue_S2(j + 2);
             }
             if (elect_one()) mma_commit(&bars[B_AB]);
             __syncwarp();
@@ -405,6 +406,22 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         auto warp_arrive = [&](int bar) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[bar]);
+        };
+        // rows 128 m .. 128 m + 127 of the W pieces -> TMEM (A operand of S'): group 0 stages pieces 0 and 1, group 1 piece 2
+        auto stage_wt = [&](int m) {
+            const int fr = 128 * m + t;
+            const uint32_t rowoff = (uint32_t)((fr & 7) * 16 + (fr >> 3) * 128);
+            for (int i = grp ? 2 : 0; i < (grp ? 3 : 2); ++i) {
+                uint32_t v[32];
+#pragma unroll
+                for (int kg = 0; kg < 8; ++kg) {
+                    uint4 w = make_uint4(0u, 0u, 0u, 0u);
+                    if (fr < NF) w = *reinterpret_cast<const uint4*>(ws_p + i * WS_BYTES + rowoff + kg * WS_SB);
+                    v[4 * kg] = w.x; v[4 * kg + 1] = w.y; v[4 * kg + 2] = w.z; v[4 * kg + 3] = w.w;
+                }
+                tmem_st32(lane_base + T_WT + 32 * i, v);
+            }
+            tmem_wait_st();
         };
         uint32_t sq = 0;                                 // ring sequence number of this tile's first slot
         bool first = true;
@@ -447,6 +464,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(hp3[4 * gq], hp3[4 * gq + 1], hp3[4 * gq + 2], hp3[4 * gq + 3]);
             }
             if (grp < KH) release(sq + grp);
+            if (proj) { stage_wt(0); tc_fence_before(); }        // (the previous tile's MMAs are complete: B_AB)
             fence_proxy_async();
             warp_arrive(B_HS);
             TRE(4);
@@ -534,32 +552,37 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(p3[0], p3[1], p3[2], p3[3]);
                 }
             }
+            stage_wt(0);                                 // H-phase TMEM buffers are dead (B_ND): W tile 0 for S'
             fence_proxy_async();
             tc_fence_before();
             warp_arrive(B_HS2);
             TRE(7);
             }   // !proj
 
-            // ---- W phase: super-chunk j = chunks 2j + grp; thread = (frames t and 128 + t, 16 pixels) ----
+            // ---- W phase: M tile m, super-chunk j = chunks 2j + grp; thread = (frame 128 m + t, 16 pixels) ----
             pending = false;
-            for (int j = 0; j < NSC2; ++j) {
-                const int c = 2 * j + grp;
-                const uint32_t seq = sq + KH + (proj ? 0 : NC) + 2 * c;
-                TRE(200 + j);
-                const unsigned char* xsl = wait_full(seq);
-                const unsigned char* osl = wait_full(seq + 1);
-                TRE(210 + j);
-                for (int m = 0; m < MT; ++m) {
-                    const int fr = 128 * m + t;
-                    const bool active = 128 * m + 32 * q < N;        // warp-uniform: some lane has a frame
+            for (int m = 0; m < MT; ++m) {
+                if (m > 0) {                             // this group's last S' wait of tile m - 1 is behind it: restage W
+                    stage_wt(m);
+                    tc_fence_before();
+                    warp_arrive(B_WT);
+                }
+                const int fr = 128 * m + t;
+                const bool active = 128 * m + 32 * q < N;            // warp-uniform: some lane has a frame
+                for (int j = 0; j < NSC2; ++j) {
+                    const int c = 2 * j + grp;
+                    const uint32_t seq = sq + KH + NCR + NCH2 * m + c;
+                    TRE(200 + j);
+                    const unsigned char* xsl = wait_full(seq);       // X rows at +0, Omega rows at +8 KB
+                    TRE(210 + j);
                     float x[16], o[16];
                     if (active) {
                         if (fr < N) {
-                            const int sw = (fr >> 1) & 3;
+                            const int sw = (t >> 1) & 3;
 #pragma unroll
                             for (int ch = 0; ch < 4; ++ch) {
-                                const float4 xv = *reinterpret_cast<const float4*>(xsl + fr * 64 + ((ch ^ sw) << 4));
-                                const float4 ov = *reinterpret_cast<const float4*>(osl + fr * 64 + ((ch ^ sw) << 4));
+                                const float4 xv = *reinterpret_cast<const float4*>(xsl + t * 64 + ((ch ^ sw) << 4));
+                                const float4 ov = *reinterpret_cast<const float4*>(xsl + 128 * PCH * 4 + t * 64 + ((ch ^ sw) << 4));
                                 x[4 * ch] = xv.x; x[4 * ch + 1] = xv.y; x[4 * ch + 2] = xv.z; x[4 * ch + 3] = xv.w;
                                 o[4 * ch] = ov.x; o[4 * ch + 1] = ov.y; o[4 * ch + 2] = ov.z; o[4 * ch + 3] = ov.w;
                             }
@@ -568,27 +591,27 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                             for (int i = 0; i < 16; ++i) { x[i] = 0.f; o[i] = 0.f; }
                         }
                     }
-                    wait(B_S2 + 2 * (j & 1) + m); tc_fence_after();
-                    if (m == 0) TRE(220 + j);
+                    wait(B_S20 + (j & 1)); tc_fence_after();
+                    TRE(220 + j);
                     uint32_t e[32];
                     if (active) {
-                        const uint32_t zcol = lane_base + T_WZ + 32 * (2 * (j & 1) + m) + 16 * grp;
+                        const uint32_t zcol = lane_base + T_WZ + 32 * (j & 1) + 16 * grp;
                         uint32_t s[16];
                         tmem_ld16(zcol, s);
                         tmem_wait_ld();
                         ew16(x, o, s, zcol, e);
                     }
-                    if (m == 0) TRE(230 + j);
-                    if (m == 0 && pending) { wait(B_ABG0 + grp); tc_fence_after(); }
-                    if (m == 0) TRE(240 + j);
-                    if (active) tmem_st32(lane_base + T_WE + 32 * (2 * grp + m), e);
+                    release(seq);                        // after the values were consumed (see the H phase)
+                    TRE(230 + j);
+                    if (pending) { wait(B_ABG0 + grp); tc_fence_after(); }
+                    TRE(240 + j);
+                    if (active) tmem_st32(lane_base + T_WE + 32 * grp, e);
+                    tmem_wait_st();
+                    tc_fence_before();
+                    warp_arrive(B_P20 + grp);
+                    pending = true;
+                    TRE(250 + j);
                 }
-                release(seq); release(seq + 1);          // after the values were consumed (see the H phase)
-                tmem_wait_st();
-                tc_fence_before();
-                warp_arrive(B_P20 + grp);
-                pending = true;
-                TRE(250 + j);
             }
             wait(B_ABG0 + grp);
             TRE(8);
@@ -712,7 +735,7 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
     const long long trows = (long long)batch * rows;
     if (!make_map(&a.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) ||
         !make_map(&a.mXh, X, trows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om, trows, p->P, FCH, TILE, false) ||
-        !make_map(&a.mXw, X, trows, p->P, rows, PCH, true) || !make_map(&a.mOw, Om, trows, p->P, rows, PCH, true)) {
+        !make_map(&a.mXw, X, trows, p->P, 128, PCH, true) || !make_map(&a.mOw, Om, trows, p->P, 128, PCH, true)) {
         if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
         return NMF_ERR_CUDA;
     }
