@@ -294,6 +294,39 @@ def run_ours(args, rank, world, local_rank):
     print(json.dumps(line))
 
 
+def run_configs(args):
+    """--configs: fit-iteration rate of every BASELINE.json config (CUDA events around nmf_fit / nmf_fit_batched
+    on random data of each config's shape; throughput does not depend on the values).  A secondary table for
+    DESIGN.md; the driver's contract line is the default mode."""
+    import torch
+    from paper_2309_04623_b200 import nmf
+    torch.cuda.set_device(0)
+    rows = [("tiny", 1, 16, 64 * 64, 5), ("MIRI-shaped", 1, 96, 256 * 256, 30), ("STIS-shaped", 1, 200, 1024 * 1024, 50)]
+    rows += [(f"sweep K={K}", 1, 200, 1024 * 1024, K) for K in (1, 5, 10, 20, 50, 100)]
+    rows += [("survey batch (64 problems)", 64, 128, 256 * 256, 20)]
+    out = {}
+    for name, B, N, P, K in rows:
+        plan = nmf.Plan(N, P, K, batch=B)
+        shp = (lambda *d: (B, *d)) if B > 1 else (lambda *d: d)
+        X = torch.rand(shp(N, P), device="cuda") * 10
+        Om = torch.rand(shp(N, P), device="cuda"); Om = Om * (Om > 0.1)
+        W = torch.rand(shp(N, K), device="cuda") + 0.1
+        H = torch.rand(shp(K, P), device="cuda") + 0.1
+        fit = plan.fit_batched if B > 1 else plan.fit
+        iters = max(3, min(200, int(2e11 / (12.0 * B * N * K * P))))
+        fit(X, Om, W, H, 3)
+        e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        torch.cuda.synchronize()
+        e0.record(); fit(X, Om, W, H, iters); e1.record(); torch.cuda.synchronize()
+        ms = e0.elapsed_time(e1) / iters
+        F, Bt = flops_per_iter(N, P, K) * B, bytes_per_iter(N, P, K) * B
+        out[name] = {"variant": plan.variant, "ms_per_iteration": ms, "iterations_per_s": 1e3 / ms,
+                     "algorithmic_tflops": F / ms / 1e9, "algorithmic_gbs": Bt / ms / 1e6}
+        del plan, X, Om, W, H
+        torch.cuda.empty_cache()
+    print(json.dumps({"configs": out}))
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -303,12 +336,16 @@ def main():
     ap.add_argument("--workload", default="stis", choices=sorted(WORKLOADS))
     ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused FFMA, 3 tensor core")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--configs", action="store_true", help="print the fit-iteration rate of every config and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.impl == "reference":
+    if args.configs:
+        if rank == 0:
+            run_configs(args)
+    elif args.impl == "reference":
         run_reference(args, rank)
     else:
         run_ours(args, rank, world, local_rank)

@@ -2,8 +2,11 @@
 //
 // One persistent, warp-specialised CTA per SM walks tiles of 128 pixels:
 //   warps 0-7  element-wise warps, two groups of four (one thread per TMEM lane in each group)
-//   warp  8    MMA issuer (one thread issues every tcgen05.mma / tcgen05.commit)
-//   warp  9    TMA producer (one thread streams H, X and Omega tiles through a ring of 16 KB slots)
+//   warps 8-9  idle (they wait at the final barrier): with the issuer and the producer as warps 8 and 9 the
+//              element-wise warps 0 / 4 and 1 / 5 shared a scheduler with them and ran their chunks 2x slower,
+//              gating their groups; 384 threads get the same 168 registers as 320
+//   warp  10   TMA producer (one thread streams H, X and Omega tiles through a ring of 16 KB slots)
+//   warp  11   MMA issuer (one elected thread issues every tcgen05.mma / tcgen05.commit)
 // All six contractions of Eq. 3 run as tcgen05.mma kind::f16 on BF16 operands with FP32
 // accumulation in TMEM.  Every FP32 operand x is split exactly into three BF16 pieces x = x1 + x2 + x3
 // (x1 = bf16(x), x2 = bf16(x - x1), x3 = x - x1 - x2) and a product a*b is evaluated as the six piece
@@ -37,8 +40,8 @@ namespace {
 using namespace tc;
 
 constexpr int EW_WARPS = 8;
-constexpr int W_MMA = 8, W_TMA = 9;
-constexpr int CTA_THREADS = 320;
+constexpr int W_MMA = 11, W_TMA = 10;
+constexpr int CTA_THREADS = 384;
 constexpr int TILE = 128;                  // pixels per tile = UMMA M of the H phase
 constexpr int FCH = 16;                    // frames per H-phase chunk (one UMMA K step)
 constexpr int PCH = 16;                    // pixels per W-phase chunk
@@ -385,7 +388,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             TR(0, 7);
             TR_NEXT;
         }
-    } else {
+    } else if (warp < EW_WARPS) {
         // =========================== element-wise warps ===========================
         const int q = warp & 3, grp = warp >> 2;
         const int t = 32 * q + lane;                     // TMEM lane: H-phase pixel / W-phase frame in the M tile
