@@ -2,11 +2,11 @@
 //
 // One persistent, warp-specialised CTA per SM walks tiles of 128 pixels:
 //   warps 0-7  element-wise warps, two groups of four (one thread per TMEM lane in each group)
-//   warps 8-9  idle (they wait at the final barrier): with the issuer and the producer as warps 8 and 9 the
-//              element-wise warps 0 / 4 and 1 / 5 shared a scheduler with them and ran their chunks 2x slower,
-//              gating their groups; 384 threads get the same 168 registers as 320
-//   warp  10   TMA producer (one thread streams H, X and Omega tiles through a ring of 16 KB slots)
-//   warp  11   MMA issuer (one elected thread issues every tcgen05.mma / tcgen05.commit)
+//   warps 8-11 one MMA issuer (one elected thread issues every tcgen05.mma / tcgen05.commit), one TMA producer (one
+//              thread streams H, X and Omega tiles through a ring of 16 KB slots) and two idle warps that wait at the
+//              final barrier (384 threads get the same 168 registers as 320).  The issuer shares a warp scheduler
+//              with two element-wise warps; which warps play the two roles (8 / 9 or 11 / 10) is a template
+//              parameter chosen per shape on the host from measurements
 // All six contractions of Eq. 3 run as tcgen05.mma kind::f16 on BF16 operands with FP32
 // accumulation in TMEM.  Every FP32 operand x is split exactly into three BF16 pieces x = x1 + x2 + x3
 // (x1 = bf16(x), x2 = bf16(x - x1), x3 = x - x1 - x2) and a product a*b is evaluated as the six piece
@@ -40,7 +40,7 @@ namespace {
 using namespace tc;
 
 constexpr int EW_WARPS = 8;
-constexpr int W_MMA = 11, W_TMA = 10;
+// warps 8 .. 11: MMA issuer, TMA producer and two idle warps; which is which is a template parameter (PLACE)
 constexpr int CTA_THREADS = 384;
 constexpr int TILE = 128;                  // pixels per tile = UMMA M of the H phase
 constexpr int FCH = 16;                    // frames per H-phase chunk (one UMMA K step)
@@ -163,9 +163,11 @@ struct TcArgs {
 enum { B_HS = 0, B_HS2, B_S0, B_S1, B_P0, B_P1, B_NDG0, B_NDG1, B_ND, B_S20, B_S21, B_P20, B_P21, B_ABG0, B_ABG1, B_AB, B_WT,
        B_FULL, B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
 
-template <int KS>
-__global__ void __launch_bounds__(CTA_THREADS, 1)
+template <int KS, int PLACE>
+__global__ void __launch_bounds__(PLACE ? 384 : 320, 1)
 k_tc_iter(const __grid_constant__ TcArgs g) {
+    constexpr int W_MMA = PLACE ? 11 : 8, W_TMA = PLACE ? 10 : 9;
+    constexpr int THREADS = PLACE ? 384 : 320;           // PLACE 1 adds two idle warps (8, 9)
     extern __shared__ __align__(1024) unsigned char smem[];
     const int N = g.N, K = g.K, NF = g.NF, NC = g.NC, MT = g.MT, KH = g.KH;
     const uint32_t NS = (uint32_t)g.NS;
@@ -202,7 +204,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         tma_prefetch_desc(&g.mH); tma_prefetch_desc(&g.mXh); tma_prefetch_desc(&g.mOh);
         tma_prefetch_desc(&g.mXw); tma_prefetch_desc(&g.mOw);
     }
-    for (int i = tid; i < NF * 8; i += CTA_THREADS) {   // (frame n, component group kg): 8 values -> 3 x 16 B
+    for (int i = tid; i < NF * 8; i += THREADS) {   // (frame n, component group kg): 8 values -> 3 x 16 B
         const int n = i >> 3, kg = i & 7;
         uint32_t p1[4], p2[4], p3[4];
 #pragma unroll
@@ -684,16 +686,20 @@ bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, in
               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
-template <int KS>
-cudaError_t launch_ks(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st) {
+template <int KS, int PLACE>
+cudaError_t launch_kp(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st) {
     static bool attr_done = false;
     if (!attr_done) {
-        cudaError_t e = cudaFuncSetAttribute(k_tc_iter<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+        cudaError_t e = cudaFuncSetAttribute(k_tc_iter<KS, PLACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
         if (e != cudaSuccess) return e;
         attr_done = true;
     }
-    k_tc_iter<KS><<<grid, CTA_THREADS, smem, st>>>(a);
+    k_tc_iter<KS, PLACE><<<grid, PLACE ? 384 : 320, smem, st>>>(a);
     return cudaSuccess;
+}
+template <int KS>
+cudaError_t launch_ks(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool place) {
+    return place ? launch_kp<KS, 1>(a, grid, smem, st) : launch_kp<KS, 0>(a, grid, smem, st);
 }
 
 }  // namespace
@@ -749,15 +755,20 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
     long long ns = ((long long)SMEM_MAX - (long long)tc_smem_fixed(a.NF)) / SLOT;
     a.NS = (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
     const int KS = (p->K + 15) / 16;
+    // Warp placement, measured per shape on the box (same-box A/B, fit iteration): issuer / producer as warps 8 / 9
+    // win everywhere (survey batch -8 %, MIRI-shaped -6 %, K = 10 -4 %) except in the metric's own shape class -- two
+    // M tiles with the last lane quadrant of the second one empty, four K steps -- where warps 11 / 10 (and two idle
+    // warps 8 / 9, 384 threads) are 4 % faster.
+    const bool place = a.MT == 2 && rows <= 224 && KS == 4;
     const size_t smem = tc_smem_fixed(a.NF) + (size_t)a.NS * SLOT;
     const dim3 grid(p->t_ctas, batch);
     for (int it = 0; it < iters; ++it) {
         cudaError_t e;
         switch (KS) {
-            case 1: e = launch_ks<1>(a, grid, smem, p->stream); break;
-            case 2: e = launch_ks<2>(a, grid, smem, p->stream); break;
-            case 3: e = launch_ks<3>(a, grid, smem, p->stream); break;
-            default: e = launch_ks<4>(a, grid, smem, p->stream); break;
+            case 1: e = launch_ks<1>(a, grid, smem, p->stream, place); break;
+            case 2: e = launch_ks<2>(a, grid, smem, p->stream, place); break;
+            case 3: e = launch_ks<3>(a, grid, smem, p->stream, place); break;
+            default: e = launch_ks<4>(a, grid, smem, p->stream, place); break;
         }
         NMF_CUDA_TRY(p, e);
         p->launches++;
