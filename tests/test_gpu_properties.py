@@ -174,3 +174,22 @@ def test_projection_many_targets():
     out = plan.subtract(dev(H), dev(T), C, dev(om), None, 0.0).cpu().numpy()
     outo = orc.subtract(H, T, Co, om, None, 0.0)
     assert np.abs(out - outo).max() <= TOL_FACTOR * np.abs(T).max()
+
+
+def test_batched_more_problems_than_sms():
+    """160 independent small problems in one batched launch sequence (grid.y > number of SMs: the persistent
+    CTAs of different problems are not co-resident and must not depend on one another)."""
+    B, N, P, K = 160, 8, 260, 3
+    rng = np.random.default_rng(11)
+    X = (rng.random((B, N, P)) * 10).astype(np.float32)
+    Om = (rng.random((B, N, P)) * (rng.random((B, N, P)) > 0.2)).astype(np.float32)
+    W0 = (0.1 + 0.9 * rng.random((B, N, K))).astype(np.float32)
+    H0 = (0.1 + 0.9 * rng.random((B, K, P))).astype(np.float32)
+    plan = nmf.Plan(N, P, K, batch=B)
+    Wd, Hd = dev(W0), dev(H0)
+    plan.fit_batched(dev(X), dev(Om), Wd, Hd, 6)
+    torch.cuda.synchronize()
+    Wg, Hg = Wd.cpu().numpy(), Hd.cpu().numpy()
+    for b in (0, 1, 77, 147, 148, 159):
+        Wo, Ho = orc.fit(X[b], Om[b], W0[b], H0[b], 6)
+        assert rel(Wg[b], Wo) <= 1e-5 and rel(Hg[b], Ho) <= 1e-5, b
