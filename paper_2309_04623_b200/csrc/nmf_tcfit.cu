@@ -9,29 +9,31 @@
 //              parameter chosen per shape on the host from measurements
 // All six contractions of Eq. 3 run as tcgen05.mma kind::f16 on BF16 operands with FP32
 // accumulation in TMEM.  Every FP32 operand x is split exactly into three BF16 pieces x = x1 + x2 + x3
-// (x1 = bf16(x), x2 = bf16(x - x1), x3 = x - x1 - x2) and a product a*b is evaluated as the six piece
-// products a1b1 + a1b2 + a2b1 + a2b2 + a1b3 + a3b1 (dropped terms <= 2^-24 |ab|), so the arithmetic stays
+// (x1 = x to 8 significant bits, x2 = the next 8 bits, x3 = the rest) and a product a*b is evaluated as the six piece
+// products a1b1 + a1b2 + a2b1 + a2b2 + a1b3 + a3b1 (dropped terms <= 2^-22 |ab|), so the arithmetic stays
 // FP32-faithful ("BF16x3", the BF16 analogue of the 3xTF32 split; 16-bit operands can be read both K-major
 // and MN-major from one no-swizzle buffer, so W and H' serve two contractions each from one copy).
 //
 // Per tile (p0 .. p0+127), with W (3 pieces, [frames][comps]) resident in shared memory:
 //   H phase (TMEM lane = pixel), 16 frames per chunk, chunk c handled by group c & 1:
 //     H0   the H tile (TMA -> ring) is split and written to shared memory as Hs[pixel][comp]       (a1)
-//     S    S^T[pixel][frame] = Hs . Ws^T  (SS MMAs, N = 16)                                         (a2)
+//     S    S^T[pixel][frame] = Hs . Ws^T, 32 frames (two chunks) per series of SS MMAs              (a2)
 //     EW   thread = (pixel, 16 frames): X, Omega from the ring; q = Om*X (select), r = Om*S,
 //          split -> TMEM (R1, R2 overwrite S in place)                                              (a3)
 //     ND   Num^T += Q^T . W, Den^T += R^T . W   (A from TMEM, B = MN-major view of Ws)              (a4)
 //     UPD  h' = h * num / max(den, eps) -> global H and, split, back into Hs                        (a5)
-//   W phase (TMEM lane = frame, M tiles of 128 frames), 16 pixels per chunk, chunk c by group c & 1:
-//     S'   S'[frame][pixel] = Ws . Hs^T (SS MMAs, N = 16)                                           (a6)
+//   W phase (TMEM lane = frame), one M tile of 128 frames at a time, 16 pixels per chunk, chunk c by group c & 1:
+//     WT   the M tile's rows of the W pieces are staged into TMEM (tcgen05.st)
+//     S'   S'[frame][pixel] = W . Hs^T, 32 pixels per series of TS MMAs (A = W tile in TMEM: tensor rate) (a6)
 //     EW   thread = (frame, 16 pixels): X, Omega re-read (L2) through TMA (64-byte swizzled rows);
 //          q, r' = Om*S' split -> TMEM                                                              (a6)
 //     AB   A += Q . Hs, B += R' . Hs  (A from TMEM, B = MN-major view of Hs), accumulated in TMEM
 //          over all tiles of the CTA                                                                (a7)
 //   After the last tile the [2][N][64] accumulators go to this CTA's slab; nmf_launch_w_update reduces
 //   the slabs in fixed order and updates W (a8).
-// Every chunk's S / piece columns are double-buffered in TMEM (one buffer per group), so the element-wise
-// work of chunk c+1 overlaps the MMAs of chunk c, and the TMA ring runs ahead across phase and tile borders.
+// S / S' are double-buffered in TMEM per 32-frame / 32-pixel super-chunk and each group has its own piece columns, so
+// the element-wise work of one buffer overlaps the MMAs of the other, and the TMA ring runs ahead across phase and
+// tile borders.  In projection mode (nmf_project, a9) H is fixed and only H0 and the W phase run.
 #include <cuda.h>
 #include "nmf_common.cuh"
 #include "nmf_tc.cuh"
