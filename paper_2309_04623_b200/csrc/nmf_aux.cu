@@ -132,7 +132,7 @@ int nmf_aux_objective(nmf_plan* p, const float* X, const float* Om, const float*
                       double* out_host) {
     const unsigned grid = (unsigned)((p->P + OBJ_THREADS - 1) / OBJ_THREADS);
     const size_t smem = sizeof(float) * ((size_t)p->N * p->K + (size_t)p->K * OBJ_THREADS);
-    static bool attr_done = false;
+    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
     if (!attr_done) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_objective, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_done = true;

@@ -253,7 +253,7 @@ template <int KC>
 int launch(nmf_plan* p, const float* X, const float* Om, const float* W, float* H, int batch) {
     const int T = p->f_threads;
     const size_t smem = fused_smem(p->N, T, KC);
-    static bool attr_done = false;
+    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
     if (!attr_done) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_fused_iter<KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
         attr_done = true;

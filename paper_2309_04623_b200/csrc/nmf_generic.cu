@@ -305,7 +305,7 @@ int launch_h(nmf_plan* p, const float* X, const float* Om, const float* W, float
     const long long pairs_per_cta = GH_THREADS / KS;
     dim3 grid((unsigned)((p->P / 2 + pairs_per_cta - 1) / pairs_per_cta), batch);
     size_t smem = sizeof(float) * (size_t)p->N * KS * round4(KC);
-    static bool attr_done = false;
+    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
     if (!attr_done) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_h_step<KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
         attr_done = true;
@@ -322,7 +322,7 @@ int launch_w(nmf_plan* p, const float* X, const float* Om, float* W, const float
     int nfb, NBc, threads;
     w_geometry(rows, KC, KS, &nfb, &NBc, &threads);
     size_t smem = w_smem(KC, KS, NBc);
-    static bool attr_done = false;
+    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
     if (!attr_done) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_w_partial<KC, W_NF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_w_partial<KC, W_NF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));

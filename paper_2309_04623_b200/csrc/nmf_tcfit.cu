@@ -689,19 +689,19 @@ bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, in
 }
 
 template <int KS, int PLACE>
-cudaError_t launch_kp(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st) {
-    static bool attr_done = false;
-    if (!attr_done) {
+cudaError_t launch_kp(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
+    static bool attr_done[64] = {};                      // function attributes are per device
+    if (device < 0 || device >= 64 || !attr_done[device]) {
         cudaError_t e = cudaFuncSetAttribute(k_tc_iter<KS, PLACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
         if (e != cudaSuccess) return e;
-        attr_done = true;
+        if (device >= 0 && device < 64) attr_done[device] = true;
     }
     k_tc_iter<KS, PLACE><<<grid, PLACE ? 384 : 320, smem, st>>>(a);
     return cudaSuccess;
 }
 template <int KS>
-cudaError_t launch_ks(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool place) {
-    return place ? launch_kp<KS, 1>(a, grid, smem, st) : launch_kp<KS, 0>(a, grid, smem, st);
+cudaError_t launch_ks(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, bool place, int device) {
+    return place ? launch_kp<KS, 1>(a, grid, smem, st, device) : launch_kp<KS, 0>(a, grid, smem, st, device);
 }
 
 }  // namespace
@@ -767,10 +767,10 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
     for (int it = 0; it < iters; ++it) {
         cudaError_t e;
         switch (KS) {
-            case 1: e = launch_ks<1>(a, grid, smem, p->stream, place); break;
-            case 2: e = launch_ks<2>(a, grid, smem, p->stream, place); break;
-            case 3: e = launch_ks<3>(a, grid, smem, p->stream, place); break;
-            default: e = launch_ks<4>(a, grid, smem, p->stream, place); break;
+            case 1: e = launch_ks<1>(a, grid, smem, p->stream, place, p->device); break;
+            case 2: e = launch_ks<2>(a, grid, smem, p->stream, place, p->device); break;
+            case 3: e = launch_ks<3>(a, grid, smem, p->stream, place, p->device); break;
+            default: e = launch_ks<4>(a, grid, smem, p->stream, place, p->device); break;
         }
         NMF_CUDA_TRY(p, e);
         p->launches++;
