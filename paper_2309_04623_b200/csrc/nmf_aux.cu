@@ -6,13 +6,16 @@ namespace {
 
 constexpr int SUB_MC = 32;      // science frames per pass (accumulators per thread)
 constexpr int SUB_THREADS = 128;
+constexpr int SUB_MH = 16;      // frames per register pass
 constexpr int SUB_PX = 4;       // pixels per thread (one 128-bit column segment of H, T, omega, out)
 constexpr int OBJ_THREADS = 128;
 
 // out[m,p] = t[m,p] - f[m] * sum_k c[m,k] H[k,p]; `fill` where omega[m,p] == 0.
-// Four pixels per thread and up to SUB_MC frames at once: H is streamed once per pass with 128-bit loads, the
-// coefficients come as 128-bit shared-memory broadcasts (cs[k][m], four frames per load), 128 FFMA per k.
-__global__ void __launch_bounds__(SUB_THREADS, 3)
+// Four pixels per thread (128-bit loads of H, T, omega; 128-bit stores), SUB_MC frames per launch handled as
+// SUB_MC / SUB_MH passes of SUB_MH frames: 64 accumulators keep the register count near 100, so five CTAs per SM
+// overlap one another's compute (K loop) and streaming (T, omega, out) phases; the H columns of the second pass
+// come back from L1 / L2.  Coefficients are 128-bit shared-memory broadcasts (cs[k][m]).
+__global__ void __launch_bounds__(SUB_THREADS, 5)
 k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float* __restrict__ C,
            const float* __restrict__ om, const float* __restrict__ factor, float fill,
            float* __restrict__ out, int M, long long P, int K, int m0) {
@@ -25,52 +28,54 @@ k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float
     __syncthreads();
     const long long p = ((long long)blockIdx.x * SUB_THREADS + threadIdx.x) * SUB_PX;
     if (p >= P) return;                            // P % 4 == 0: a segment is all in or all out
-    float acc[SUB_MC][SUB_PX];
+    for (int mh = 0; mh < mc; mh += SUB_MH) {
+        float acc[SUB_MH][SUB_PX];
 #pragma unroll
-    for (int m = 0; m < SUB_MC; ++m)
+        for (int m = 0; m < SUB_MH; ++m)
 #pragma unroll
-        for (int q = 0; q < SUB_PX; ++q) acc[m][q] = 0.f;
-    const float* hp = H + p;
-    constexpr int KU = 5;                          // H rows in flight per thread (128-bit loads)
-    for (int k0 = 0; k0 < K; k0 += KU) {
-        float4 hv[KU];
+            for (int q = 0; q < SUB_PX; ++q) acc[m][q] = 0.f;
+        const float* hp = H + p;
+        constexpr int KU = 5;                      // H rows in flight per thread
+        for (int k0 = 0; k0 < K; k0 += KU) {
+            float4 hv[KU];
 #pragma unroll
-        for (int u = 0; u < KU; ++u)
-            hv[u] = (k0 + u < K) ? __ldg(reinterpret_cast<const float4*>(hp + (size_t)(k0 + u) * P)) : make_float4(0.f, 0.f, 0.f, 0.f);
+            for (int u = 0; u < KU; ++u)
+                hv[u] = (k0 + u < K) ? __ldg(reinterpret_cast<const float4*>(hp + (size_t)(k0 + u) * P)) : make_float4(0.f, 0.f, 0.f, 0.f);
 #pragma unroll
-        for (int u = 0; u < KU; ++u) {
-            if (k0 + u < K) {
-                const float4 h = hv[u];
-                const float* ck = cs + (k0 + u) * SUB_MC;
+            for (int u = 0; u < KU; ++u) {
+                if (k0 + u < K) {
+                    const float4 h = hv[u];
+                    const float* ck = cs + (k0 + u) * SUB_MC + mh;
 #pragma unroll
-                for (int m4 = 0; m4 < SUB_MC / 4; ++m4) {
-                    const float4 c = *reinterpret_cast<const float4*>(ck + 4 * m4);
-                    const float cc[4] = {c.x, c.y, c.z, c.w};
+                    for (int m4 = 0; m4 < SUB_MH / 4; ++m4) {
+                        const float4 c = *reinterpret_cast<const float4*>(ck + 4 * m4);
+                        const float cc[4] = {c.x, c.y, c.z, c.w};
 #pragma unroll
-                    for (int v = 0; v < 4; ++v) {
-                        acc[4 * m4 + v][0] = fmaf(cc[v], h.x, acc[4 * m4 + v][0]);
-                        acc[4 * m4 + v][1] = fmaf(cc[v], h.y, acc[4 * m4 + v][1]);
-                        acc[4 * m4 + v][2] = fmaf(cc[v], h.z, acc[4 * m4 + v][2]);
-                        acc[4 * m4 + v][3] = fmaf(cc[v], h.w, acc[4 * m4 + v][3]);
+                        for (int v = 0; v < 4; ++v) {
+                            acc[4 * m4 + v][0] = fmaf(cc[v], h.x, acc[4 * m4 + v][0]);
+                            acc[4 * m4 + v][1] = fmaf(cc[v], h.y, acc[4 * m4 + v][1]);
+                            acc[4 * m4 + v][2] = fmaf(cc[v], h.z, acc[4 * m4 + v][2]);
+                            acc[4 * m4 + v][3] = fmaf(cc[v], h.w, acc[4 * m4 + v][3]);
+                        }
                     }
                 }
             }
         }
-    }
 #pragma unroll
-    for (int m = 0; m < SUB_MC; ++m) {
-        if (m < mc) {
-            const size_t i = (size_t)(m0 + m) * P + p;
-            const float f = factor ? factor[m0 + m] : 1.f;
-            const float4 t = __ldg(reinterpret_cast<const float4*>(T + i));
-            float4 o = make_float4(1.f, 1.f, 1.f, 1.f);
-            if (om) o = __ldg(reinterpret_cast<const float4*>(om + i));
-            float4 r;                              // omega == 0: T may hold NaN/Inf there (G5) -> select
-            r.x = o.x > 0.f ? t.x - f * acc[m][0] : fill;
-            r.y = o.y > 0.f ? t.y - f * acc[m][1] : fill;
-            r.z = o.z > 0.f ? t.z - f * acc[m][2] : fill;
-            r.w = o.w > 0.f ? t.w - f * acc[m][3] : fill;
-            *reinterpret_cast<float4*>(out + i) = r;
+        for (int m = 0; m < SUB_MH; ++m) {
+            if (mh + m < mc) {
+                const size_t i = (size_t)(m0 + mh + m) * P + p;
+                const float f = factor ? factor[m0 + mh + m] : 1.f;
+                const float4 t = __ldg(reinterpret_cast<const float4*>(T + i));
+                float4 o = make_float4(1.f, 1.f, 1.f, 1.f);
+                if (om) o = __ldg(reinterpret_cast<const float4*>(om + i));
+                float4 r;                          // omega == 0: T may hold NaN/Inf there (G5) -> select
+                r.x = o.x > 0.f ? t.x - f * acc[m][0] : fill;
+                r.y = o.y > 0.f ? t.y - f * acc[m][1] : fill;
+                r.z = o.z > 0.f ? t.z - f * acc[m][2] : fill;
+                r.w = o.w > 0.f ? t.w - f * acc[m][3] : fill;
+                *reinterpret_cast<float4*>(out + i) = r;
+            }
         }
     }
 }
