@@ -174,3 +174,42 @@ void oracle_subtract(int M, long P, int K, const double* H, const float* T,
         }
     }
 }
+
+/* ---- closest-frame reference selection ------------- */
+/* "The target PSFs are then compared to the reference library, and a
+ * percentage of the closest frames ... are selected.  The closest frames are
+ * calculated by minimizing for Euclidean norm".  Readings (G19, G20):
+ *   D[m,n] = sum over the pixels that are valid in BOTH frames (om_t[m,p] > 0 and
+ *            Om[n,p] > 0; masked regions are "missing data and ignored",
+ *            PAPER.md:81) of (T[m,p] - X[n,p])^2      -- squared Euclidean distance;
+ *   the n_sel closest references of target m are the n_sel smallest D[m,:], ties
+ *   broken by the lower frame index, listed in ascending order of (D, index).
+ * The percentage itself is the caller's choice (the paper gives no formula).
+ * Pins: tests/test_oracle_pins.py (brute force, identities, masks, ties).        */
+void oracle_ref_distance(int M, int N, long P, const float* T, const float* om_t /* nullable */,
+                         const float* X, const float* Om /* nullable */, double* D /* [M,N] */) {
+#pragma omp parallel for schedule(static) collapse(2)
+    for (int m = 0; m < M; ++m)
+        for (int n = 0; n < N; ++n) {
+            double s = 0.0;
+            for (long p = 0; p < P; ++p) {
+                if (om_t && !((double)om_t[(size_t)m * P + p] > 0.0)) continue;
+                if (Om && !((double)Om[(size_t)n * P + p] > 0.0)) continue;
+                const double d = (double)T[(size_t)m * P + p] - (double)X[(size_t)n * P + p];
+                s += d * d;
+            }
+            D[(size_t)m * N + n] = s;
+        }
+}
+
+void oracle_ref_select(int M, int N, const double* D, int n_sel, int* idx /* [M,n_sel] */) {
+    for (int m = 0; m < M; ++m) {
+        const double* d = D + (size_t)m * N;
+        for (int n = 0; n < N; ++n) {            /* rank of n under the order (D, index) */
+            int rank = 0;
+            for (int j = 0; j < N; ++j)
+                if (d[j] < d[n] || (d[j] == d[n] && j < n)) ++rank;
+            if (rank < n_sel) idx[(size_t)m * n_sel + rank] = n;
+        }
+    }
+}

@@ -47,6 +47,8 @@ def _load():
                                        ctypes.c_int]
         lib.oracle_subtract.argtypes = [ctypes.c_int, ctypes.c_long, ctypes.c_int, _D, _F, _D, _F,
                                         _D, ctypes.c_double, _D]
+        lib.oracle_ref_distance.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_long, _F, _F, _F, _F, _D]
+        lib.oracle_ref_select.argtypes = [ctypes.c_int, ctypes.c_int, _D, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         _lib = lib
     return _lib
 
@@ -126,6 +128,30 @@ def subtract(H, T, C, omega_t=None, factor=None, fill: float = 0.0):
     out = np.empty((M, P), dtype=np.float64)
     _load().oracle_subtract(M, P, K, hp, tp, cp, op, fp, float(fill), out.ctypes.data_as(_D))
     return out
+
+
+def ref_distance(T, omega_t, X, Omega):
+    """Masked squared Euclidean distances D[m,n] between targets T [M,P] and references X [N,P] (fp64);
+    pixels with omega_t[m,p] == 0 or Omega[n,p] == 0 are skipped."""
+    T, tp = _f32(T); X, xp = _f32(X)
+    M, P = T.shape; N = X.shape[0]
+    otp = op = None
+    if omega_t is not None:
+        ot, otp = _f32(omega_t)
+    if Omega is not None:
+        om, op = _f32(Omega)
+    D = np.empty((M, N), dtype=np.float64)
+    _load().oracle_ref_distance(M, N, P, tp, otp, xp, op, D.ctypes.data_as(_D))
+    return D
+
+
+def ref_select(D, n_sel: int):
+    """Indices [M,n_sel] of the n_sel closest references per target, ascending in (distance, index)."""
+    D, dp = _f64(D)
+    M, N = D.shape
+    idx = np.full((M, n_sel), -1, dtype=np.int32)
+    _load().oracle_ref_select(M, N, dp, int(n_sel), idx.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
+    return idx
 
 
 if __name__ == "__main__":

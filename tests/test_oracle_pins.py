@@ -287,3 +287,80 @@ def test_generator_structure():
     s = inputs.make_stis(N=3, S=128, K=4, M=1)
     frac = float((s.Omega[0] == 0).mean())
     assert 0.05 < frac < 0.08
+
+
+# ---------------------------------------------------------------------------------------------
+# P13-P16: closest-frame reference selection (readings G19/G20)
+# ---------------------------------------------------------------------------------------------
+def _ref_case(M=5, N=9, P=37, seed=0, masks=True):
+    rng = np.random.default_rng(seed)
+    T = (rng.random((M, P)) * 4).astype(np.float32)
+    X = (rng.random((N, P)) * 4).astype(np.float32)
+    ot = (rng.random((M, P)) > 0.3).astype(np.float32) * (0.5 + rng.random((M, P))).astype(np.float32) if masks else None
+    Om = (rng.random((N, P)) > 0.2).astype(np.float32) * (0.5 + rng.random((N, P))).astype(np.float32) if masks else None
+    return T, ot, X, Om
+
+
+def test_p13_ref_distance_brute_force_and_expansion():
+    """D against (a) pure-Python loops on a tiny case and (b) the expanded form
+    sum a b t^2 - 2 sum (a t)(b x) + sum a b x^2 (three matrix products with the 0/1 masks a, b)."""
+    T, ot, X, Om = _ref_case()
+    D = orc.ref_distance(T, ot, X, Om)
+    M, N, P = T.shape[0], X.shape[0], T.shape[1]
+    for m in range(M):
+        for n in range(N):
+            s = 0.0
+            for p in range(P):
+                if ot[m, p] > 0 and Om[n, p] > 0:
+                    s += (float(T[m, p]) - float(X[n, p])) ** 2
+            assert abs(D[m, n] - s) <= 1e-12 * max(s, 1.0)
+    a, b = (ot > 0).astype(np.float64), (Om > 0).astype(np.float64)
+    t, x = T.astype(np.float64), X.astype(np.float64)
+    E = (a * t * t) @ b.T - 2.0 * (a * t) @ (b * x).T + a @ (b * x * x).T
+    assert np.abs(D - E).max() <= 1e-10 * np.abs(E).max()
+
+
+def test_p14_ref_distance_identities():
+    T, ot, X, Om = _ref_case(M=4, N=6, P=50, seed=3)
+    X[2] = T[1]                                    # a reference equal to a target: distance 0 on any mask
+    D = orc.ref_distance(T, ot, X, Om)
+    assert D[1, 2] == 0.0 and (D >= 0).all()
+    # symmetry: swapping the roles transposes D
+    assert np.array_equal(orc.ref_distance(X, Om, T, ot), D.T)
+    # no masks: the plain squared Euclidean norm; NULL == all-ones masks
+    Dn = orc.ref_distance(T, None, X, None)
+    assert np.allclose(Dn, ((T[:, None, :].astype(np.float64) - X[None].astype(np.float64)) ** 2).sum(-1), rtol=1e-13)
+    assert np.array_equal(Dn, orc.ref_distance(T, np.ones_like(T), X, np.ones_like(X)))
+    # scaling both by s scales D by s^2; a common offset leaves it unchanged (exact in fp64 for powers of two)
+    assert np.array_equal(orc.ref_distance(T * np.float32(4), ot, X * np.float32(4), Om), D * 16.0)
+    # every masked pair contributes nothing: masking a pixel can only lower D
+    ot2 = ot.copy(); ot2[:, ::3] = 0
+    assert (orc.ref_distance(T, ot2, X, Om) <= D + 1e-15).all()
+
+
+def test_p15_ref_distance_mask_invariance():
+    """Masked entries may hold NaN / Inf / 1e30: bitwise the same distances."""
+    T, ot, X, Om = _ref_case(seed=5)
+    D = orc.ref_distance(T, ot, X, Om)
+    for g in (np.nan, np.inf, 1e30):
+        T2, X2 = T.copy(), X.copy()
+        T2[ot == 0] = g; X2[Om == 0] = g
+        assert np.array_equal(orc.ref_distance(T2, ot, X2, Om), D)
+
+
+def test_p16_ref_select_order_and_ties():
+    rng = np.random.default_rng(9)
+    D = rng.random((6, 40))
+    D[2, 7] = D[2, 31] = D[2].min() / 2            # an exact tie for first place: lower index first
+    D[4] = 1.0                                     # all equal: identity order
+    for n_sel in (1, 5, 40):
+        idx = orc.ref_select(D, n_sel)
+        ref = np.argsort(D, axis=1, kind="stable")[:, :n_sel]
+        assert np.array_equal(idx, ref)
+    assert list(orc.ref_select(D, 2)[2]) == [7, 31]
+    assert list(orc.ref_select(D, 3)[4]) == [0, 1, 2]
+    # selecting the closest frames of a library that contains the target itself returns it first
+    T, ot, X, Om = _ref_case(M=3, N=8, P=64, seed=1)
+    X[5] = T[0]; X[1] = T[2]
+    idx = orc.ref_select(orc.ref_distance(T, ot, X, Om), 4)
+    assert idx[0, 0] == 5 and idx[2, 0] == 1
