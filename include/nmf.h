@@ -142,6 +142,28 @@ int nmf_project_subtract_host(nmf_plan* plan, const float* H_dev, const float* t
                               const float* omega_host, float* coef_host, float fill,
                               float* out_host, int M, int iters);
 
+/* Closest-frame reference selection ("a percentage of the closest
+ * frames ... calculated by minimizing for Euclidean norm"; readings G19/G20 in
+ * DESIGN.md).  nmf_ref_distance writes the masked squared Euclidean distances
+ *   dist[m,n] = sum over pixels with omega_t[m,p] > 0 and Omega[n,p] > 0 of
+ *               (target[m,p] - X[n,p])^2
+ * between M target frames and the plan's N library frames (masked entries are
+ * skipped and may hold NaN/Inf).  Partial sums are fp32 per pixel
+ * range and reduced in fp64 in a fixed order (bitwise reproducible).
+ *   target device [M,P]   omega_t device [M,P] or NULL = all valid
+ *   X      device [N,P]   Omega   device [N,P] or NULL = all valid
+ *   dist   device [M,N]   out (fp32, 16-byte aligned)
+ * M is not limited by max_targets.  Errors: INVALID_ARG, ALIGNMENT, WORKSPACE, CUDA. */
+int nmf_ref_distance(nmf_plan* plan, const float* target, const float* omega_t, const float* X,
+                     const float* Omega, int M, float* dist);
+
+/* For every target m the n_sel (1 <= n_sel <= N) references with the smallest
+ * dist[m,:], in ascending order of (distance, frame index) -- the percentage of
+ * the library to keep is the caller's choice (the paper gives no formula).
+ *   dist device [M,N] read-only     idx device [M,n_sel] out (int32)
+ * Errors: INVALID_ARG, CUDA.                                                       */
+int nmf_ref_select(nmf_plan* plan, const float* dist, int M, int n_sel, int* idx);
+
 /* Number of kernel launches this plan has enqueued so far (bench bookkeeping).     */
 long long nmf_plan_launch_count(const nmf_plan* plan);
 

@@ -11,8 +11,10 @@ size_t plan_workspace(nmf_plan* p) {
     size_t g = nmf_generic_workspace(p);
     size_t f = nmf_fused_workspace(p);
     size_t t = nmf_tc_workspace(p);
+    size_t sel = nmf_select_workspace(p);
     if (f > g) g = f;
     if (t > g) g = t;
+    if (sel > g) g = sel;
     size_t main = nmf_align_up(g, 256);
     return main + nmf_align_up(nmf_aux_workspace(p), 256);
 }
@@ -223,6 +225,25 @@ int nmf_project_subtract_host(nmf_plan* p, const float* H, const float* Th, cons
     NMF_CUDA_TRY(p, cudaMemcpyAsync(outh, out, sizeof(float) * (size_t)M * p->P, cudaMemcpyDeviceToHost, p->stream));
     NMF_CUDA_TRY(p, cudaStreamSynchronize(p->stream));
     return NMF_OK;
+}
+
+int nmf_ref_distance(nmf_plan* p, const float* T, const float* ot, const float* X, const float* Om, int M,
+                     float* dist) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!T || !X || !dist || M < 1) return NMF_ERR_INVALID_ARG;
+    if (misaligned(T) || misaligned(X) || misaligned(dist) || (ot && misaligned(ot)) || (Om && misaligned(Om)))
+        return NMF_ERR_ALIGNMENT;
+    int rc = check_ws(p);
+    if (rc) return rc;
+    return nmf_select_distance(p, T, ot, X, Om, M, dist);
+}
+
+int nmf_ref_select(nmf_plan* p, const float* dist, int M, int n_sel, int* idx) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!dist || !idx || M < 1 || n_sel < 1 || n_sel > p->N) return NMF_ERR_INVALID_ARG;
+    return nmf_select_topn(p, dist, M, n_sel, idx);
 }
 
 long long nmf_plan_launch_count(const nmf_plan* p) { return p ? p->launches : 0; }

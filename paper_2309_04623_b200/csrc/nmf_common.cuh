@@ -82,6 +82,11 @@ int    nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float*
                   int iters, int batch);
 int    nmf_tc_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C,
                       int M, int iters);
+// closest-frame reference selection (nmf_select.cu)
+size_t nmf_select_workspace(const nmf_plan* p);
+int    nmf_select_distance(nmf_plan* p, const float* T, const float* ot, const float* X, const float* Om,
+                           int M, float* D);
+int    nmf_select_topn(nmf_plan* p, const float* D, int M, int n_sel, int* idx);
 // auxiliaries
 size_t nmf_aux_workspace(const nmf_plan* p);
 int    nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C,

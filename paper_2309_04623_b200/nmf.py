@@ -24,6 +24,7 @@ SYMBOLS = (
     "nmf_plan_create", "nmf_plan_workspace_bytes", "nmf_plan_set_workspace", "nmf_plan_set_stream",
     "nmf_plan_set_variant", "nmf_plan_get_variant", "nmf_plan_destroy", "nmf_fit", "nmf_fit_batched",
     "nmf_project", "nmf_subtract", "nmf_objective", "nmf_fit_host", "nmf_project_subtract_host",
+    "nmf_ref_distance", "nmf_ref_select",
     "nmf_plan_launch_count", "nmf_status_string", "nmf_plan_last_cuda_error",
 )
 
@@ -58,6 +59,8 @@ def lib():
         L.nmf_project.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci]
         L.nmf_subtract.argtypes = [_vp, _vp, _vp, _vp, _vp, _vp, _cf, _vp, _ci]
         L.nmf_objective.argtypes = [_vp, _vp, _vp, _vp, _vp, ctypes.POINTER(ctypes.c_double)]
+        L.nmf_ref_distance.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
+        L.nmf_ref_select.argtypes = [_vp, _vp, _ci, _ci, _vp]
         L.nmf_fit_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci]
         L.nmf_project_subtract_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _cf, _vp, _ci, _ci]
         L.nmf_plan_launch_count.argtypes = [_vp]; L.nmf_plan_launch_count.restype = _cll
@@ -159,6 +162,27 @@ class Plan:
                                        None if factor is None else _dev(factor, (M,)),
                                        float(fill), _dev(out, (M, self.P)), M))
         return out
+
+    def ref_distance(self, target, omega_t, X, Omega, out=None):
+        """nmf_ref_distance: masked squared Euclidean distances [M,N] (fp32, device) between M targets and X."""
+        M = target.shape[0]
+        if out is None:
+            out = torch.empty((M, self.N), dtype=torch.float32, device=self.device)
+        self._sync_stream()
+        self._check(lib().nmf_ref_distance(self._h, _dev(target, (M, self.P)),
+                                           None if omega_t is None else _dev(omega_t, (M, self.P)),
+                                           _dev(X, (self.N, self.P)),
+                                           None if Omega is None else _dev(Omega, (self.N, self.P)),
+                                           M, _dev(out, (M, self.N))))
+        return out
+
+    def ref_select(self, dist, n_sel: int):
+        """nmf_ref_select: int32 [M,n_sel] indices of the n_sel closest references per target."""
+        M = dist.shape[0]
+        idx = torch.empty((M, n_sel), dtype=torch.int32, device=self.device)
+        self._sync_stream()
+        self._check(lib().nmf_ref_select(self._h, _dev(dist, (M, self.N)), M, int(n_sel), idx.data_ptr()))
+        return idx
 
     def objective(self, X, Omega, W, H) -> float:
         out = ctypes.c_double(0.0)

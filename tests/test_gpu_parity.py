@@ -110,3 +110,53 @@ def test_projection_omega_null_and_factor():
     outo = orc.subtract(H, p.T, C.cpu().numpy(), None, fac)
     assert np.abs(out - outo).max() <= 1e-5 * np.abs(p.T).max()
     assert np.array_equal(out[0], p.T[0])
+
+
+# ---- closest-frame reference selection ------------------------------------
+def _check_ref_selection(T, ot, X, Om, n_sel, K=4):
+    M, P = T.shape; N = X.shape[0]
+    plan = nmf.Plan(N, P, K)
+    d = lambda a: None if a is None else dev(a)
+    Dg = plan.ref_distance(d(T), d(ot), d(X), d(Om))
+    idx = plan.ref_select(Dg, n_sel)
+    torch.cuda.synchronize()
+    Dg, idx = Dg.cpu().numpy(), idx.cpu().numpy()
+    Do = orc.ref_distance(T, ot, X, Om)
+    assert np.all(np.isfinite(Dg))
+    assert np.abs(Dg - Do).max() <= 1e-5 * np.abs(Do).max()           # fp32 partials, fp64 fixed-order reduce
+    # the selection is an integer decision: bit-exact against the oracle's rule applied to the same fp32 distances
+    assert np.array_equal(idx, orc.ref_select(Dg.astype(np.float64), n_sel))
+    # and it is a valid answer for the fp64 distances: what it picks is as close as what the oracle picks
+    pick = np.take_along_axis(Do, idx.astype(np.int64), axis=1)
+    best = np.sort(Do, axis=1)[:, :n_sel]
+    assert np.all(np.abs(pick - best) <= 2e-5 * np.abs(Do).max())
+    return Dg, idx
+
+
+@pytest.mark.parametrize("M,N,P", [(1, 1, 4), (5, 9, 36), (33, 130, 1028), (40, 200, 4100), (3, 256, 516)])
+def test_ref_selection_ragged(M, N, P):
+    rng = np.random.default_rng(M * 100 + N)
+    T = (rng.random((M, P)) * 4).astype(np.float32)
+    X = (rng.random((N, P)) * 4).astype(np.float32)
+    ot = ((rng.random((M, P)) > 0.3) * (0.5 + rng.random((M, P)))).astype(np.float32)
+    Om = ((rng.random((N, P)) > 0.2) * (0.5 + rng.random((N, P)))).astype(np.float32)
+    if N > 2:
+        X[N // 2] = T[0]                                   # the library contains target 0: it must come first
+        Om[N // 2] = 1.0
+    Dg, idx = _check_ref_selection(T, ot, X, Om, max(1, N // 3))
+    if N > 2:
+        assert idx[0, 0] == N // 2 and Dg[0, N // 2] == 0.0
+    # garbage in masked entries changes nothing, bitwise
+    T2, X2 = T.copy(), X.copy()
+    T2[ot == 0] = np.nan; X2[Om == 0] = np.inf
+    plan = nmf.Plan(N, P, 4)
+    D2 = plan.ref_distance(dev(T2), dev(ot), dev(X2), dev(Om)).cpu().numpy()
+    assert np.array_equal(D2, Dg)
+    # NULL masks = all valid
+    _check_ref_selection(T, None, X, None, 1)
+
+
+def test_ref_selection_stis_shaped():
+    """Science frames against the STIS-shaped library at 200 frames x 192^2 px: keep the closest 30 %."""
+    p = inputs.make_stis(S=192, M=8)
+    _check_ref_selection(p.T, p.omega_t, p.X, p.Omega, int(0.3 * p.N), K=p.K)
