@@ -34,35 +34,57 @@ k_ref_dist(const float* __restrict__ T, const float* __restrict__ ot, const floa
     const long long p_hi = p_lo + px_per_cta < P ? p_lo + px_per_cta : P;
     const int mi = threadIdx.x >> 5, ni = threadIdx.x & 31;     // targets 4 mi + i, references ni + 32 j
     const float qnan = __int_as_float(0x7fc00000);
-    float acc[4][4];
+    float acc[4][4], tot[4][4];
 #pragma unroll
     for (int i = 0; i < 4; ++i)
 #pragma unroll
-        for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
+        for (int j = 0; j < 4; ++j) tot[i][j] = 0.f;
 
-    for (long long pt = p_lo; pt < p_hi; pt += SD_TP) {
-        // stage: row r of the block, pixel column c; masked or out-of-range entries become NaN
-        for (int i = threadIdx.x; i < (SD_MB + SD_NB) * SD_TP; i += SD_THREADS) {
-            const int r = i >> 5, c = i & 31;
-            const long long p = pt + c;
-            float v = qnan;
-            if (r < SD_MB) {
-                const int m = m0 + r;
-                if (m < M && p < p_hi) {
-                    const size_t g = (size_t)m * P + p;
-                    if (!ot || ot[g] > 0.f) v = T[g];
-                }
-                ts[r][c] = v;
-            } else {
-                const int n = n0 + r - SD_MB;
-                if (n < N && p < p_hi) {
-                    const size_t g = (size_t)n * P + p;
-                    if (!Om || Om[g] > 0.f) v = X[g];
-                }
-                xs[r - SD_MB][c] = v;
+    // staging: (SD_MB + SD_NB) rows x 8 float4 per tile = SD_LOADS float4 per thread and array, prefetched one tile
+    // ahead into registers (values and masks are loaded unconditionally and independently, then selected)
+    constexpr int SD_LOADS = (SD_MB + SD_NB) * (SD_TP / 4) / SD_THREADS;     // 5
+    float4 rv[SD_LOADS], rm[SD_LOADS];
+    auto fetch = [&](long long pt) {
+#pragma unroll
+        for (int u = 0; u < SD_LOADS; ++u) {
+            const int i = threadIdx.x + u * SD_THREADS;
+            const int r = i >> 3, c4 = i & 7;
+            const long long p = pt + 4 * c4;
+            const bool is_t = r < SD_MB;
+            const int row = is_t ? m0 + r : n0 + r - SD_MB;
+            const bool ok = p < p_hi && (is_t ? row < M : row < N);          // P % 4 == 0: all four or none
+            const float* val = is_t ? T : X;
+            const float* msk = is_t ? ot : Om;
+            rv[u] = make_float4(qnan, qnan, qnan, qnan);
+            rm[u] = make_float4(1.f, 1.f, 1.f, 1.f);
+            if (ok) {
+                const size_t g = (size_t)row * P + p;
+                rv[u] = __ldg(reinterpret_cast<const float4*>(val + g));
+                if (msk) rm[u] = __ldg(reinterpret_cast<const float4*>(msk + g));
             }
         }
+    };
+    auto stash = [&]() {                                    // masked entries become NaN
+#pragma unroll
+        for (int u = 0; u < SD_LOADS; ++u) {
+            const int i = threadIdx.x + u * SD_THREADS;
+            const int r = i >> 3, c4 = i & 7;
+            float4 v;
+            v.x = rm[u].x > 0.f ? rv[u].x : qnan; v.y = rm[u].y > 0.f ? rv[u].y : qnan;
+            v.z = rm[u].z > 0.f ? rv[u].z : qnan; v.w = rm[u].w > 0.f ? rv[u].w : qnan;
+            float* dst = r < SD_MB ? &ts[r][4 * c4] : &xs[r - SD_MB][4 * c4];
+            *reinterpret_cast<float4*>(dst) = v;
+        }
+    };
+    if (p_lo < p_hi) fetch(p_lo);
+    for (long long pt = p_lo; pt < p_hi; pt += SD_TP) {
+        stash();
         __syncthreads();
+        if (pt + SD_TP < p_hi) fetch(pt + SD_TP);           // in flight during the compute of this tile
+#pragma unroll
+        for (int i = 0; i < 4; ++i)
+#pragma unroll
+            for (int j = 0; j < 4; ++j) acc[i][j] = 0.f;
 #pragma unroll 2
         for (int c = 0; c < SD_TP; c += 4) {
             float4 tv[4], xv[4];
@@ -81,6 +103,10 @@ k_ref_dist(const float* __restrict__ T, const float* __restrict__ ot, const floa
                     d = tv[i].w - xv[j].w; acc[i][j] += fmaxf(d * d, 0.f);
                 }
         }
+#pragma unroll
+        for (int i = 0; i < 4; ++i)                          // two-level sum: short fp32 chains
+#pragma unroll
+            for (int j = 0; j < 4; ++j) tot[i][j] += acc[i][j];
         __syncthreads();
     }
     // partial slab of this pixel range: [part][SD_MB][N]
@@ -90,7 +116,7 @@ k_ref_dist(const float* __restrict__ T, const float* __restrict__ ot, const floa
 #pragma unroll
         for (int j = 0; j < 4; ++j) {
             const int n = n0 + ni + 32 * j;
-            if (n < N) out[(size_t)(4 * mi + i) * N + n] = acc[i][j];
+            if (n < N) out[(size_t)(4 * mi + i) * N + n] = tot[i][j];
         }
 }
 

@@ -160,3 +160,9 @@ def test_ref_selection_stis_shaped():
     """Science frames against the STIS-shaped library at 200 frames x 192^2 px: keep the closest 30 %."""
     p = inputs.make_stis(S=192, M=8)
     _check_ref_selection(p.T, p.omega_t, p.X, p.Omega, int(0.3 * p.N), K=p.K)
+
+
+def test_ref_selection_full_size():
+    """Full STIS-shaped library (200 frames x 1024^2 px), 4 science frames: every distance against the oracle."""
+    p = inputs.make_stis(M=4)
+    _check_ref_selection(p.T, p.omega_t, p.X, p.Omega, 60, K=p.K)
