@@ -1,12 +1,12 @@
-// nmf_tc.cuh -- sm_100a primitives used by the tensor-core NMF kernels (inline PTX only):
-// mbarrier, proxy/tcgen05 fences, TMEM allocation, tcgen05.ld/st, UMMA shared-memory and
-// instruction descriptors, tcgen05.mma (kind::tf32, A from shared memory or from TMEM) and commit.
+// nmf_tc.cuh -- sm_100a primitives used by the tensor-core NMF kernel (inline PTX only):
+// mbarrier, TMA (cp.async.bulk.tensor), proxy/tcgen05 fences, TMEM allocation, tcgen05.ld/st, the UMMA
+// shared-memory descriptor and tcgen05.commit.  (The kind::f16 MMA wrappers live next to the kernel.)
 //
-// Operand layouts (no-swizzle "interleaved" canonical form, 32-bit elements, T = 4 per 16 bytes):
-//   a buffer Z[a][b] is stored as 8x4 core matrices (8 consecutive a, 4 consecutive b, 128 bytes):
-//       byte(a, b) = (a % 8) * 16 + (a / 8) * SA + (b % 4) * 4 + (b / 4) * SB
-//   * read as a K-major operand   (MN = a, K = b): SBO = SA, LBO = SB, one MMA (K = 8) spans 2 LBO
-//   * read as an MN-major operand (MN = b, K = a): SBO = SB, LBO = SA, one MMA (K = 8) spans 1 group
+// Operand layout (no-swizzle canonical form, 16-bit elements, 8 per 16 bytes):
+//   a buffer Z[a][b] is stored as 8x8 core matrices (8 consecutive a, 8 consecutive b, 128 bytes):
+//       byte(a, b) = (a % 8) * 16 + (a / 8) * 128 + (b % 8) * 2 + (b / 8) * SB
+//   * read as a K-major operand   (MN = a, K = b): SBO = 128, LBO = SB, one MMA (K = 16) spans 2 LBO
+//   * read as an MN-major operand (MN = b, K = a): SBO = SB, LBO = 128, one MMA (K = 16) spans 2 row groups
 // so the same bytes serve W (frames x components) and H^T (pixels x components) in both roles.
 #pragma once
 #include <cuda_runtime.h>
@@ -117,37 +117,9 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes
     return (uint64_t)((saddr >> 4) & 0x3FFFu) | ((uint64_t)((lbo_bytes >> 4) & 0x3FFFu) << 16) |
            ((uint64_t)((sbo_bytes >> 4) & 0x3FFFu) << 32) | (1ull << 46);
 }
-// instruction descriptor, kind::tf32, fp32 accumulate, M in {64,128}, N % 16 == 0 (M = 128)
-__host__ __device__ constexpr uint32_t idesc_tf32(int M, int N, int a_mn_major, int b_mn_major) {
-    return (1u << 4) | (2u << 7) | (2u << 10) | ((uint32_t)a_mn_major << 15) | ((uint32_t)b_mn_major << 16) |
-           ((uint32_t)(N >> 3) << 17) | ((uint32_t)(M >> 4) << 24);
-}
-
-// ---------------------------------------------------------------- MMA issue (one thread)
-__device__ __forceinline__ void mma_ss(uint32_t d_tmem, uint64_t a_desc, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], %1, %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "l"(a_desc), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
-}
-__device__ __forceinline__ void mma_ts(uint32_t d_tmem, uint32_t a_tmem, uint64_t b_desc, uint32_t idesc, uint32_t acc) {
-    asm volatile(
-        "{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-        "tcgen05.mma.cta_group::1.kind::tf32 [%0], [%1], %2, %3, p;\n\t}"
-        ::"r"(d_tmem), "r"(a_tmem), "l"(b_desc), "r"(idesc), "r"(acc) : "memory");
-}
 // all previously issued MMAs of this thread arrive on `bar` when complete (implies fence::before_thread_sync)
 __device__ __forceinline__ void mma_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
-}
-
-// ---------------------------------------------------------------- fp32 -> (hi, lo) TF32 split
-// hi = x rounded to 10 explicit mantissa bits (nearest), lo = x - hi (exact in fp32); the tensor core reads
-// the top 19 bits of lo.  x*y ~= hi_x*hi_y + lo_x*hi_y + hi_x*lo_y with relative error ~2^-21.
-__device__ __forceinline__ void split_tf32(float x, uint32_t& hi, uint32_t& lo) {
-    const uint32_t h = (__float_as_uint(x) + 0x1000u) & 0xFFFFE000u;
-    hi = h;
-    lo = __float_as_uint(x - __uint_as_float(h));
 }
 
 }  // namespace tc
