@@ -143,8 +143,8 @@ int nmf_project(nmf_plan* p, const float* H, const float* T, const float* om, fl
     int rc = check_ws(p);
     if (rc) return rc;
     if (iters == 0) return NMF_OK;
-    // tensor-core W phase with H fixed when the plan's fit runs there too
-    if (pick_variant(p) == 3) return nmf_tc_project(p, H, T, om, C, M, iters);
+    // tensor-core W phase with H fixed when the plan's fit runs there too (omega == NULL: generic path)
+    if (om && pick_variant(p) == 3) return nmf_tc_project(p, H, T, om, C, M, iters);
     return nmf_generic_project(p, H, T, om, C, M, iters);
 }
 

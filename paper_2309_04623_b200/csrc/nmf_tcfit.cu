@@ -158,7 +158,6 @@ struct TcArgs {
     int MT;                    // 128-frame M tiles of the W phase (1 or 2)
     int KH;                    // 32-component slots of the H tile (1 or 2)
     int NS;                    // ring slots
-    int om_null;               // 1: projection without weights (omega == NULL: all ones, nothing masked)
     int proj;                  // 1: projection (a9): H is fixed, only the W phase runs (X = targets, Om = omega, W = coef)
 };
 
@@ -263,10 +262,9 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 }
                 for (int m = 0; m < MT; ++m)             // W phase: M tile m's 128 rows of X and Omega, 16 px at a time
                     for (int c = 0; c < NCH2; ++c) {
-                        const uint32_t s = acquire((g.om_null ? 1 : 2) * 128 * PCH * 4);
+                        const uint32_t s = acquire(2 * 128 * PCH * 4);
                         tma_load_2d(ring_s + s * SLOT, &g.mXw, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
-                        if (!g.om_null)
-                            tma_load_2d(ring_s + s * SLOT + 128 * PCH * 4, &g.mOw, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
+                        tma_load_2d(ring_s + s * SLOT + 128 * PCH * 4, &g.mOw, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
                     }
             }
         }
@@ -591,8 +589,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
 #pragma unroll
                             for (int ch = 0; ch < 4; ++ch) {
                                 const float4 xv = *reinterpret_cast<const float4*>(xsl + t * 64 + ((ch ^ sw) << 4));
-                                float4 ov = make_float4(1.f, 1.f, 1.f, 1.f);          // omega == NULL: every weight is 1 ...
-                                if (!g.om_null) ov = *reinterpret_cast<const float4*>(xsl + 128 * PCH * 4 + t * 64 + ((ch ^ sw) << 4));
+                                const float4 ov = *reinterpret_cast<const float4*>(xsl + 128 * PCH * 4 + t * 64 + ((ch ^ sw) << 4));
                                 x[4 * ch] = xv.x; x[4 * ch + 1] = xv.y; x[4 * ch + 2] = xv.z; x[4 * ch + 3] = xv.w;
                                 o[4 * ch] = ov.x; o[4 * ch + 1] = ov.y; o[4 * ch + 2] = ov.z; o[4 * ch + 3] = ov.w;
                             }
@@ -748,15 +745,15 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
     TcArgs a;
     const long long trows = (long long)batch * rows;
     if (!make_map(&a.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) ||
-        !make_map(&a.mXh, X, trows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om ? Om : X, trows, p->P, FCH, TILE, false) ||
-        !make_map(&a.mXw, X, trows, p->P, 128, PCH, true) || !make_map(&a.mOw, Om ? Om : X, trows, p->P, 128, PCH, true)) {
+        !make_map(&a.mXh, X, trows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om, trows, p->P, FCH, TILE, false) ||
+        !make_map(&a.mXw, X, trows, p->P, 128, PCH, true) || !make_map(&a.mOw, Om, trows, p->P, 128, PCH, true)) {
         if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
         return NMF_ERR_CUDA;
     }
     a.W = W; a.H = const_cast<float*>(H); a.slab = reinterpret_cast<float*>(p->ws);
     a.N = rows; a.K = p->K; a.P = p->P; a.n_tiles = (p->P + TILE - 1) / TILE;
     a.NF = (rows + FCH - 1) / FCH * FCH; a.NC = a.NF / FCH; a.MT = (rows + 127) / 128;
-    a.KH = (p->K + 31) / 32; a.proj = proj ? 1 : 0; a.om_null = Om ? 0 : 1;
+    a.KH = (p->K + 31) / 32; a.proj = proj ? 1 : 0;
     long long ns = ((long long)SMEM_MAX - (long long)tc_smem_fixed(a.NF)) / SLOT;
     a.NS = (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
     const int KS = (p->K + 15) / 16;
@@ -793,11 +790,10 @@ int nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
 // Projection (a9) on the tensor cores: the W phase alone with H fixed, X = targets, Omega = omega, W = coef.
 // Frames are handled 256 at a time (the W phase holds two 128-row M tiles).
 int nmf_tc_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C, int M, int iters) {
-    if (!p->t_ctas) return NMF_ERR_UNSUPPORTED;
+    if (!p->t_ctas || !om) return NMF_ERR_UNSUPPORTED;
     for (int m0 = 0; m0 < M; m0 += 256) {
         const int rows = M - m0 < 256 ? M - m0 : 256;
-        int rc = tc_run(p, T + (size_t)m0 * p->P, om ? om + (size_t)m0 * p->P : nullptr, C + (size_t)m0 * p->K, H, rows,
-                        iters, 1, true);
+        int rc = tc_run(p, T + (size_t)m0 * p->P, om + (size_t)m0 * p->P, C + (size_t)m0 * p->K, H, rows, iters, 1, true);
         if (rc) return rc;
     }
     return NMF_OK;
