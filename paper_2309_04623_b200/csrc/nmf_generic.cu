@@ -236,22 +236,24 @@ k_w_partial(const float* __restrict__ X, const float* __restrict__ Om, const flo
 // ---------------------------------------------------------------------------
 // Fixed-order reduction of the partial slabs (fp64) + W <- W o A / max(B, eps)
 // ---------------------------------------------------------------------------
-// 256 threads = 8 part lanes x 32 elements: lane q sums the parts q, q + 8, ... in order, the 8 partial sums are
-// then added in lane order -- a fixed association, so the result is bitwise reproducible.
-__global__ void __launch_bounds__(256)
+// 256 threads = 32 part lanes x 8 elements: lane q sums the parts q, q + 32, ... in order (independent loads, at most
+// five per thread for 148 slabs), the 32 partial sums are then added in lane order -- a fixed association, so the
+// result is bitwise reproducible.
+constexpr int WU_E = 8, WU_Q = 32;
+__global__ void __launch_bounds__(WU_E * WU_Q)
 k_w_update(const float* __restrict__ slab, float* __restrict__ W, int N, int K, int KT, int parts) {
-    __shared__ double sa[8][32], sd[8][32];
+    __shared__ double sa[WU_Q][WU_E], sd[WU_Q][WU_E];
     const int b = blockIdx.y;
-    const int e = threadIdx.x & 31, q = threadIdx.x >> 5;
-    const int i = blockIdx.x * 32 + e;
+    const int e = threadIdx.x % WU_E, q = threadIdx.x / WU_E;
+    const int i = blockIdx.x * WU_E + e;
     const bool ok = i < N * K;
     const int n = ok ? i / K : 0, k = ok ? i - n * K : 0;
     const size_t stride = (size_t)2 * N * KT;
     const float* s = slab + (size_t)b * parts * stride + (size_t)n * KT + k;
     double a = 0.0, d = 0.0;
     if (ok) {
-#pragma unroll 4
-        for (int part = q; part < parts; part += 8) {
+#pragma unroll 5
+        for (int part = q; part < parts; part += WU_Q) {
             a += (double)s[(size_t)part * stride];
             d += (double)s[(size_t)part * stride + (size_t)N * KT];
         }
@@ -260,7 +262,7 @@ k_w_update(const float* __restrict__ slab, float* __restrict__ W, int N, int K, 
     __syncthreads();
     if (q == 0 && ok) {
 #pragma unroll
-        for (int r = 1; r < 8; ++r) { a += sa[r][e]; d += sd[r][e]; }
+        for (int r = 1; r < WU_Q; ++r) { a += sa[r][e]; d += sd[r][e]; }
         float* w = W + (size_t)b * N * K + i;
         *w = (*w * (float)a) / fmaxf((float)d, NMF_EPS);
     }
@@ -334,8 +336,8 @@ int launch_w(nmf_plan* p, const float* X, const float* Om, float* W, const float
         k_w_partial<KC, W_NF, true><<<grid, threads, smem, p->stream>>>(X, Om, W, H, slab, rows, p->P, p->K, KS, NBc);
     else
         k_w_partial<KC, W_NF, false><<<grid, threads, smem, p->stream>>>(X, Om, W, H, slab, rows, p->P, p->K, KS, NBc);
-    dim3 g2((rows * p->K + 31) / 32, batch);
-    k_w_update<<<g2, 256, 0, p->stream>>>(slab, W, rows, p->K, KC * KS, parts);
+    dim3 g2((rows * p->K + WU_E - 1) / WU_E, batch);
+    k_w_update<<<g2, WU_E * WU_Q, 0, p->stream>>>(slab, W, rows, p->K, KC * KS, parts);
     p->launches += 2;
     return NMF_OK;
 }
@@ -384,8 +386,8 @@ size_t nmf_generic_workspace(const nmf_plan* p) {
 
 int nmf_launch_w_update(nmf_plan* p, const float* slab, float* W, int rows, int K, int KT, int parts,
                         int batch) {
-    dim3 g2((rows * K + 31) / 32, batch);
-    k_w_update<<<g2, 256, 0, p->stream>>>(slab, W, rows, K, KT, parts);
+    dim3 g2((rows * K + WU_E - 1) / WU_E, batch);
+    k_w_update<<<g2, WU_E * WU_Q, 0, p->stream>>>(slab, W, rows, K, KT, parts);
     p->launches++;
     return NMF_OK;
 }
