@@ -4,9 +4,10 @@
 //   warps 0-7  element-wise warps, two groups of four (one thread per TMEM lane in each group)
 //   warps 8-11 one MMA issuer (one elected thread issues every tcgen05.mma / tcgen05.commit), one TMA producer (one
 //              thread streams H, X and Omega tiles through a ring of 16 KB slots) and two idle warps that wait at the
-//              final barrier (384 threads get the same 168 registers as 320).  The issuer shares a warp scheduler
-//              with two element-wise warps; which warps play the two roles (8 / 9 or 11 / 10) is a template
-//              parameter chosen per shape on the host from measurements
+//              final barrier (384 threads get the same 168 registers as 320).  Whether the CTA carries the two
+//              idle warps (PLACE = 1: 384 threads, roles on warps 11 / 10) or not (PLACE = 0: 320 threads, roles on
+//              warps 8 / 9) is a template parameter chosen per shape on the host from measurements: with 384
+//              threads every role assignment measured the same, the thread count is what matters
 // All six contractions of Eq. 3 run as tcgen05.mma kind::f16 on BF16 operands with FP32
 // accumulation in TMEM.  Every FP32 operand x is split exactly into three BF16 pieces x = x1 + x2 + x3
 // (x1 = x to 8 significant bits, x2 = the next 8 bits, x3 = the rest) and a product a*b is evaluated as the six piece
@@ -757,10 +758,10 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
     long long ns = ((long long)SMEM_MAX - (long long)tc_smem_fixed(a.NF)) / SLOT;
     a.NS = (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
     const int KS = (p->K + 15) / 16;
-    // Warp placement, measured per shape on the box (same-box A/B, fit iteration): issuer / producer as warps 8 / 9
-    // win everywhere (survey batch -8 %, MIRI-shaped -6 %, K = 10 -4 %) except in the metric's own shape class -- two
-    // M tiles with the last lane quadrant of the second one empty, four K steps -- where warps 11 / 10 (and two idle
-    // warps 8 / 9, 384 threads) are 4 % faster.
+    // CTA size, measured per shape on the box (same-box A/B, fit iteration): 320 threads (issuer / producer as warps
+    // 8 / 9) win everywhere (survey batch -8 %, MIRI-shaped -6 %, K = 10 -4 %) except in the metric's own shape class
+    // -- two M tiles with the last lane quadrant of the second one empty, four K steps -- where 384 threads (two
+    // idle warps; any role assignment among warps 8 .. 11 measures the same) are 4 % faster.
     const bool place = a.MT == 2 && rows <= 224 && KS == 4;
     const size_t smem = tc_smem_fixed(a.NF) + (size_t)a.NS * SLOT;
     const dim3 grid(p->t_ctas, batch);
