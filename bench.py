@@ -50,7 +50,7 @@ def bytes_per_iter(N, P, K):
 # clocks sampler (nvidia-smi during the timed region)
 # ------------------------------------------------------------------------------
 class ClockSampler:
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
          "clocks_event_reasons.sw_power_cap")
 
@@ -63,7 +63,8 @@ class ClockSampler:
         except Exception:
             self.p = None
 
-    def stop(self):
+    def stop(self, t0=None, t1=None):
+        import datetime
         if self.p is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
         self.p.terminate()
@@ -74,23 +75,31 @@ class ClockSampler:
         self.f.flush(); self.f.seek(0)
         sm, smax, reasons, power = [], [], set(), []
         names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        rows = []
         for line in self.f:
             t = [c.strip() for c in line.split(",")]
-            if len(t) < 7:
+            if len(t) < 8:
                 continue
             try:
-                sm.append(float(t[0])); smax.append(float(t[1])); power.append(float(t[2]))
+                ts = datetime.datetime.strptime(t[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                rows.append((ts, float(t[1]), float(t[2]), float(t[3]), t[4:8]))
             except ValueError:
                 continue
-            for nm, v in zip(names, t[3:7]):
+        inside = [r for r in rows if t0 is None or (t0 - 0.02 <= r[0] <= t1 + 0.02)]
+        window = "timed region"
+        if not inside:                      # region shorter than the sampling period: the samples closest to it
+            inside = sorted(rows, key=lambda r: abs(r[0] - (t0 or 0)))[:3]
+            window = "nearest samples (timed region shorter than the sampling period)"
+        for ts, a, b, c, flags in inside:
+            sm.append(a); smax.append(b); power.append(c)
+            for nm, v in zip(names, flags):
                 if v.lower().startswith("active"):
                     reasons.add(nm)
         os.unlink(self.f.name)
-        # keep the samples taken under load (upper half of the clock readings)
         return {"sm_mhz": statistics.median(sm) if sm else None,
                 "sm_max_mhz": max(smax) if smax else None,
                 "power_w_max": max(power) if power else None,
-                "samples": len(sm), "reasons": sorted(reasons)}
+                "samples": len(sm), "window": window, "reasons": sorted(reasons)}
 
 
 # ------------------------------------------------------------------------------
@@ -154,6 +163,9 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.set_device(local_rank)
     if world > 1:
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+    # nvidia-smi needs a few hundred ms for its first sample: start it now, keep only the samples whose time stamp
+    # falls inside the timed region
+    sampler = ClockSampler(local_rank) if rank == 0 else None
     wl = WORKLOADS[args.workload]
     # every rank fits its own replica (per-rank seed): independent problems, no collective
     p = inputs.make_stis(N=wl["N"], S=wl["S"], K=wl["K"], M=wl["M"], seed=sharding.replica_seed(3003, rank))
@@ -179,8 +191,8 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    sampler = ClockSampler(local_rank) if rank == 0 else None
     l0 = plan.launch_count
+    t_wall0 = time.time()
     e0.record()
     for s in range(args.steps):
         fit_ev[s][0].record()
@@ -192,7 +204,7 @@ def run_ours(args, rank, world, local_rank):
     torch.cuda.synchronize()
     if world > 1:
         dist.barrier()
-    clocks = sampler.stop() if sampler else None
+    clocks = sampler.stop(t_wall0, time.time()) if sampler else None
     launches = plan.launch_count - l0
     ms_total = e0.elapsed_time(e1)
     fit_ms = [a.elapsed_time(b) for a, b in fit_ev]
