@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnmf_b200.so")
-SOURCES = ["nmf_api.cu", "nmf_generic.cu", "nmf_fused.cu", "nmf_tcfit.cu", "nmf_aux.cu", "nmf_select.cu"]
+SOURCES = ["nmf_api.cu", "nmf_generic.cu", "nmf_fused.cu", "nmf_tcfit.cu", "nmf_tcsplit.cu", "nmf_aux.cu", "nmf_select.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
@@ -28,12 +28,12 @@ def _deps():
     return max(os.path.getmtime(h) for h in hdrs)
 
 
-def _compile(src: str, force: bool, verbose: bool) -> str:
-    obj = os.path.join(OBJ, src.replace(".cu", ".o"))
+def _compile(src: str, force: bool, verbose: bool, extra=(), suffix: str = "") -> str:
+    obj = os.path.join(OBJ, src.replace(".cu", suffix + ".o"))
     srcp = os.path.join(CSRC, src)
     if not force and os.path.exists(obj) and os.path.getmtime(obj) >= max(os.path.getmtime(srcp), _deps()):
         return obj
-    cmd = ["nvcc", *NVCC_FLAGS, "-c", srcp, "-o", obj]
+    cmd = ["nvcc", *NVCC_FLAGS, *extra, "-c", srcp, "-o", obj]
     if verbose:
         cmd.insert(1, "-Xptxas=-v")
     r = subprocess.run(cmd, capture_output=True, text=True)
@@ -54,6 +54,19 @@ def build(force: bool = False, verbose: bool = False) -> str:
                                "-o", tmp, *objs, "-cudart", "static", "-lcuda"])
         os.replace(tmp, LIB)
     return LIB
+
+
+def build_trace() -> str:
+    """libnmf_trace.so: the same library with the tile-timeline instrumentation of nmf_tcfit.cu compiled in
+    (-DNMF_TC_TRACE; exports nmf_debug_tc_trace).  Used by `python bench.py --trace` only."""
+    os.makedirs(OBJ, exist_ok=True)
+    lib = os.path.join(OBJ, "libnmf_trace.so")
+    with cf.ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
+        objs = list(ex.map(lambda s: _compile(s, False, False, ("-DNMF_TC_TRACE",), ".trace"), SOURCES))
+    if not os.path.exists(lib) or os.path.getmtime(lib) < max(os.path.getmtime(o) for o in objs):
+        subprocess.check_call(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a",
+                               "-o", lib, *objs, "-cudart", "static", "-lcuda"])
+    return lib
 
 
 if __name__ == "__main__":

@@ -11,6 +11,8 @@ size_t plan_workspace(nmf_plan* p) {
     size_t g = nmf_generic_workspace(p);
     size_t f = nmf_fused_workspace(p);
     size_t t = nmf_tc_workspace(p);
+    size_t ts = nmf_tcsplit_workspace(p);
+    if (ts > t) t = ts;
     size_t sel = nmf_select_workspace(p);
     if (f > g) g = f;
     if (t > g) g = t;
@@ -24,12 +26,14 @@ int check_ws(const nmf_plan* p) {
     return NMF_OK;
 }
 
-// 0 auto: tensor core > fused FFMA > generic
+// 0 auto: fused tensor core (K <= 64) > split tensor core (K <= 128) > fused FFMA > generic
 int pick_variant(const nmf_plan* p) {
     if (p->variant_req == 1) return 1;
     if (p->variant_req == 2) return nmf_fused_available(p) ? 2 : 1;
+    if (p->variant_req == 4) return nmf_tcsplit_available(p) ? 4 : 1;
     if (nmf_tc_available(p)) return 3;
     if (p->variant_req == 3) return 1;
+    if (nmf_tcsplit_available(p)) return 4;
     return nmf_fused_available(p) ? 2 : 1;
 }
 
@@ -43,7 +47,9 @@ int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
     if (iters == 0) return NMF_OK;
     if (p->variant_req == 2 && !nmf_fused_available(p)) return NMF_ERR_UNSUPPORTED;
     if (p->variant_req == 3 && !nmf_tc_available(p)) return NMF_ERR_UNSUPPORTED;
+    if (p->variant_req == 4 && !nmf_tcsplit_available(p)) return NMF_ERR_UNSUPPORTED;
     const int v = pick_variant(p);
+    if (v == 4) return nmf_tcsplit_fit(p, X, Om, W, H, iters, batch);
     if (v == 3) return nmf_tc_fit(p, X, Om, W, H, iters, batch);
     if (v == 2) return nmf_fused_fit(p, X, Om, W, H, iters, batch);
     return nmf_generic_fit(p, X, Om, W, H, iters, batch);
@@ -86,6 +92,7 @@ int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int ma
     nmf_generic_configure(p);
     nmf_fused_configure(p);
     nmf_tc_configure(p);
+    nmf_tcsplit_configure(p);
     p->ws_needed = plan_workspace(p);
     *out = p;
     return NMF_OK;
@@ -108,7 +115,7 @@ int nmf_plan_set_stream(nmf_plan* p, void* s) {
 }
 
 int nmf_plan_set_variant(nmf_plan* p, int v) {
-    if (!p || v < 0 || v > 3) return NMF_ERR_INVALID_ARG;
+    if (!p || v < 0 || v > 4) return NMF_ERR_INVALID_ARG;
     p->variant_req = v;
     return NMF_OK;
 }
@@ -145,6 +152,7 @@ int nmf_project(nmf_plan* p, const float* H, const float* T, const float* om, fl
     if (iters == 0) return NMF_OK;
     // tensor-core W phase with H fixed when the plan's fit runs there too (omega == NULL: generic path)
     if (om && pick_variant(p) == 3) return nmf_tc_project(p, H, T, om, C, M, iters);
+    if (om && pick_variant(p) == 4) return nmf_tcsplit_project(p, H, T, om, C, M, iters);
     return nmf_generic_project(p, H, T, om, C, M, iters);
 }
 

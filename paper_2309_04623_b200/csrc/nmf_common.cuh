@@ -21,7 +21,7 @@ struct nmf_plan {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     size_t ws_needed = 0;
-    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 tensor core
+    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core
     long long launches = 0;
     int sticky = 0;               // first CUDA error seen (nmf_status)
     std::string cuda_msg;
@@ -37,8 +37,8 @@ struct nmf_plan {
     int f_fpw = 0;                // frames per warp in the W half
     // tensor-core path geometry (see nmf_tcfit.cu)
     int t_ctas = 0;               // persistent CTAs per problem (0 = unavailable)
-    int t_nst = 0;                // cp.async sub-stage depth of the W phase
-    bool t_attr_done = false;
+    // split tensor-core path (see nmf_tcsplit.cu)
+    bool s_ok = false;
     // host staging for the *_host entry points (plan-owned device buffers)
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -82,6 +82,14 @@ int    nmf_tc_fit(nmf_plan* p, const float* X, const float* Om, float* W, float*
                   int iters, int batch);
 int    nmf_tc_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C,
                       int M, int iters);
+// split tensor-core path: H half-step kernel + W half-step kernel, K <= 128 (nmf_tcsplit.cu)
+void   nmf_tcsplit_configure(nmf_plan* p);
+size_t nmf_tcsplit_workspace(const nmf_plan* p);
+bool   nmf_tcsplit_available(const nmf_plan* p);
+int    nmf_tcsplit_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
+                       int iters, int batch);
+int    nmf_tcsplit_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C,
+                           int M, int iters);
 // closest-frame reference selection (nmf_select.cu)
 size_t nmf_select_workspace(const nmf_plan* p);
 int    nmf_select_distance(nmf_plan* p, const float* T, const float* ot, const float* X, const float* Om,

@@ -9,6 +9,7 @@
 //   * read as an MN-major operand (MN = b, K = a): SBO = SB, LBO = 128, one MMA (K = 16) spans 2 row groups
 // so the same bytes serve W (frames x components) and H^T (pixels x components) in both roles.
 #pragma once
+#include <cuda.h>
 #include <cuda_runtime.h>
 #include <stdint.h>
 
@@ -108,6 +109,10 @@ __device__ __forceinline__ void tmem_st8(uint32_t taddr, const uint32_t (&r)[8])
                  ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7])
                  : "memory");
 }
+__device__ __forceinline__ void tmem_st4(uint32_t taddr, const uint32_t (&r)[4]) {
+    asm volatile("tcgen05.st.sync.aligned.32x32b.x4.b32 [%0], {%1,%2,%3,%4};"
+                 ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]) : "memory");
+}
 __device__ __forceinline__ void tmem_wait_ld() { asm volatile("tcgen05.wait::ld.sync.aligned;" ::: "memory"); }
 __device__ __forceinline__ void tmem_wait_st() { asm volatile("tcgen05.wait::st.sync.aligned;" ::: "memory"); }
 
@@ -120,6 +125,111 @@ __device__ __forceinline__ uint64_t smem_desc(uint32_t saddr, uint32_t lbo_bytes
 // all previously issued MMAs of this thread arrive on `bar` when complete (implies fence::before_thread_sync)
 __device__ __forceinline__ void mma_commit(uint64_t* bar) {
     asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+
+// ---------------------------------------------------------------- kind::f16 MMA (BF16 operands, FP32 accumulation)
+__host__ __device__ constexpr uint32_t idesc_bf16(int M, int N, int b_mn_major) {
+    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
+           ((uint32_t)(M >> 4) << 24);
+}
+__device__ __forceinline__ void mma16_ss(uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
+                 ::"r"(d), "l"(a), "l"(b), "r"(id), "r"(acc) : "memory");
+}
+__device__ __forceinline__ void mma16_ts(uint32_t d, uint32_t a, uint64_t b, uint32_t id, uint32_t acc) {
+    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
+                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
+                 ::"r"(d), "r"(a), "l"(b), "r"(id), "r"(acc) : "memory");
+}
+
+__device__ __forceinline__ bool elect_one() {
+    uint32_t p;
+    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
+    return p != 0;
+}
+
+// exact 3-way BF16 split of two FP32 values, packed (low half = first value): x = x1 + x2 + x3 with
+// x1 = x rounded to 8 significant bits (half away from zero), x2 = the next 8 bits of the remainder (truncated),
+// x3 = what is left (at most 8 significant bits, so it is a BF16 number).  Integer / FADD / PRMT only: the
+// F2FP conversion pipe is a quarter-rate unit and was the limiter of the element-wise warps.
+__device__ __forceinline__ void split3_pair(float x0, float x1, uint32_t& p1, uint32_t& p2, uint32_t& p3) {
+    const uint32_t a0 = (__float_as_uint(x0) + 0x8000u) & 0xffff0000u;
+    const uint32_t a1 = (__float_as_uint(x1) + 0x8000u) & 0xffff0000u;
+    const float r0 = x0 - __uint_as_float(a0);
+    const float r1 = x1 - __uint_as_float(a1);
+    const uint32_t b0 = __float_as_uint(r0) & 0xffff0000u;
+    const uint32_t b1 = __float_as_uint(r1) & 0xffff0000u;
+    const float s0 = r0 - __uint_as_float(b0);
+    const float s1 = r1 - __uint_as_float(b1);
+    p1 = __byte_perm(a0, a1, 0x7632);
+    p2 = __byte_perm(b0, b1, 0x7632);
+    p3 = __byte_perm(__float_as_uint(s0), __float_as_uint(s1), 0x7632);
+}
+
+__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
+    asm volatile(
+        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
+        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
+        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
+          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
+          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
+          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
+        : "memory");
+}
+
+
+// ---------------------------------------------------------------- element-wise stage shared by the tensor-core kernels
+// layout of a group's E buffer (32 TMEM columns): R3, Q1, Q2, Q3, 8 columns (16 BF16 values) each
+constexpr uint32_t O_R3 = 0, O_Q1 = 8, O_Q2 = 16, O_Q3 = 24;
+// q = Om*X, r = Om*S for 16 consecutive elements (Omega == 0: missing datum, skipped (G5); X may be NaN/Inf
+// there), split into BF16 pieces.  R1, R2 go back over S in place (`zcol`, this thread's lane); R3 and the Q pieces
+// are returned packed in `e` for the single-buffered E columns.
+__device__ __forceinline__ void ew16(const float (&x)[16], const float (&o)[16], const uint32_t (&s)[16], uint32_t zcol,
+                                     uint32_t (&e)[32]) {
+    uint32_t R1[8], R2[8];
+#pragma unroll
+    for (int i = 0; i < 8; ++i) {
+        const float o0 = o[2 * i], o1 = o[2 * i + 1];
+        const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
+        const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
+        const float r0 = o0 * __uint_as_float(s[2 * i]);          // S is finite: Omega == 0 gives exactly 0
+        const float r1 = o1 * __uint_as_float(s[2 * i + 1]);
+        split3_pair(q0, q1, e[O_Q1 + i], e[O_Q2 + i], e[O_Q3 + i]);
+        split3_pair(r0, r1, R1[i], R2[i], e[O_R3 + i]);
+    }
+    tmem_st8(zcol, R1); tmem_st8(zcol + 8, R2);
+}
+
+// ---------------------------------------------------------------- host: tensor maps
+// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency)
+typedef CUresult (*encode_fn_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
+                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
+                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
+
+inline encode_fn_t encode_fn() {
+    static encode_fn_t fn = nullptr;
+    if (!fn) {
+        void* p = nullptr;
+        cudaDriverEntryPointQueryResult qr;
+        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
+            qr == cudaDriverEntryPointSuccess)
+            fn = reinterpret_cast<encode_fn_t>(p);
+    }
+    return fn;
+}
+
+// 2-D fp32 map over a row-major [rows, P] array, box [box_rows][box_px]
+inline bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, int box_rows, int box_px, bool swizzle64) {
+    encode_fn_t fn = encode_fn();
+    if (!fn) return false;
+    const cuuint64_t dims[2] = {(cuuint64_t)P, (cuuint64_t)rows};
+    const cuuint64_t strides[1] = {(cuuint64_t)P * sizeof(float)};
+    const cuuint32_t box[2] = {(cuuint32_t)box_px, (cuuint32_t)box_rows};
+    const cuuint32_t estr[2] = {1, 1};
+    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
+              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 
 }  // namespace tc

@@ -44,7 +44,6 @@ using namespace tc;
 
 constexpr int EW_WARPS = 8;
 // warps 8 .. 11: MMA issuer, TMA producer and two idle warps; which is which is a template parameter (PLACE)
-constexpr int CTA_THREADS = 384;
 constexpr int TILE = 128;                  // pixels per tile = UMMA M of the H phase
 constexpr int FCH = 16;                    // frames per H-phase chunk (one UMMA K step)
 constexpr int PCH = 16;                    // pixels per W-phase chunk
@@ -65,88 +64,6 @@ constexpr uint32_t T_WE = 64;              //   E[g] at T_WE + 32 g
 constexpr uint32_t T_WT = 128;             //   the M tile's rows of W as TMEM A operand: piece i at T_WT + 32 i (comps 2c, 2c+1
                                            //   in column c), so the S' MMAs read A from TMEM and run at the tensor rate
 constexpr uint32_t T_ACC = 256;            // A_acc[m] at T_ACC + 128 m, B_acc[m] at + 64 (persistent over tiles)
-constexpr uint32_t O_R3 = 0, O_Q1 = 8, O_Q2 = 16, O_Q3 = 24;   // inside an E buffer
-
-__host__ __device__ constexpr uint32_t idesc_bf16(int M, int N, int b_mn_major) {
-    return (1u << 4) | (1u << 7) | (1u << 10) | ((uint32_t)b_mn_major << 16) | ((uint32_t)(N >> 3) << 17) |
-           ((uint32_t)(M >> 4) << 24);
-}
-__device__ __forceinline__ void mma16_ss(uint32_t d, uint64_t a, uint64_t b, uint32_t id, uint32_t acc) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::f16 [%0], %1, %2, %3, p;\n\t}"
-                 ::"r"(d), "l"(a), "l"(b), "r"(id), "r"(acc) : "memory");
-}
-__device__ __forceinline__ void mma16_ts(uint32_t d, uint32_t a, uint64_t b, uint32_t id, uint32_t acc) {
-    asm volatile("{\n\t.reg .pred p;\n\tsetp.ne.b32 p, %4, 0;\n\t"
-                 "tcgen05.mma.cta_group::1.kind::f16 [%0], [%1], %2, %3, p;\n\t}"
-                 ::"r"(d), "r"(a), "l"(b), "r"(id), "r"(acc) : "memory");
-}
-
-__device__ __forceinline__ bool elect_one() {
-    uint32_t p;
-    asm volatile("{\n\t.reg .pred P;\n\telect.sync _|P, 0xffffffff;\n\tselp.u32 %0, 1, 0, P;\n\t}" : "=r"(p));
-    return p != 0;
-}
-
-// exact 3-way BF16 split of two FP32 values, packed (low half = first value): x = x1 + x2 + x3 with
-// x1 = x rounded to 8 significant bits (half away from zero), x2 = the next 8 bits of the remainder (truncated),
-// x3 = what is left (at most 8 significant bits, so it is a BF16 number).  Integer / FADD / PRMT only: the
-// F2FP conversion pipe is a quarter-rate unit and was the limiter of the element-wise warps.
-__device__ __forceinline__ void split3_pair(float x0, float x1, uint32_t& p1, uint32_t& p2, uint32_t& p3) {
-    const uint32_t a0 = (__float_as_uint(x0) + 0x8000u) & 0xffff0000u;
-    const uint32_t a1 = (__float_as_uint(x1) + 0x8000u) & 0xffff0000u;
-    const float r0 = x0 - __uint_as_float(a0);
-    const float r1 = x1 - __uint_as_float(a1);
-    const uint32_t b0 = __float_as_uint(r0) & 0xffff0000u;
-    const uint32_t b1 = __float_as_uint(r1) & 0xffff0000u;
-    const float s0 = r0 - __uint_as_float(b0);
-    const float s1 = r1 - __uint_as_float(b1);
-    p1 = __byte_perm(a0, a1, 0x7632);
-    p2 = __byte_perm(b0, b1, 0x7632);
-    p3 = __byte_perm(__float_as_uint(s0), __float_as_uint(s1), 0x7632);
-}
-
-// q = Om*X, r = Om*S for 16 consecutive elements (Omega == 0: missing datum, skipped (G5); X may be NaN/Inf
-// there), split into BF16 pieces.  R1, R2 go back over S in place (`zcol`, this thread's lane); R3 and the Q pieces
-// are returned packed in `e` for the single-buffered E columns.
-__device__ __forceinline__ void ew16(const float (&x)[16], const float (&o)[16], const uint32_t (&s)[16], uint32_t zcol,
-                                     uint32_t (&e)[32]) {
-    uint32_t R1[8], R2[8];
-#pragma unroll
-    for (int i = 0; i < 8; ++i) {
-        const float o0 = o[2 * i], o1 = o[2 * i + 1];
-        const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
-        const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
-        const float r0 = o0 * __uint_as_float(s[2 * i]);          // S is finite: Omega == 0 gives exactly 0
-        const float r1 = o1 * __uint_as_float(s[2 * i + 1]);
-        split3_pair(q0, q1, e[O_Q1 + i], e[O_Q2 + i], e[O_Q3 + i]);
-        split3_pair(r0, r1, R1[i], R2[i], e[O_R3 + i]);
-    }
-    tmem_st8(zcol, R1); tmem_st8(zcol + 8, R2);
-}
-__device__ __forceinline__ void tmem_st32(uint32_t taddr, const uint32_t (&r)[32]) {
-    asm volatile(
-        "tcgen05.st.sync.aligned.32x32b.x32.b32 [%0], {%1,%2,%3,%4,%5,%6,%7,%8,%9,%10,%11,%12,%13,%14,%15,%16,"
-        "%17,%18,%19,%20,%21,%22,%23,%24,%25,%26,%27,%28,%29,%30,%31,%32};"
-        ::"r"(taddr), "r"(r[0]), "r"(r[1]), "r"(r[2]), "r"(r[3]), "r"(r[4]), "r"(r[5]), "r"(r[6]), "r"(r[7]),
-          "r"(r[8]), "r"(r[9]), "r"(r[10]), "r"(r[11]), "r"(r[12]), "r"(r[13]), "r"(r[14]), "r"(r[15]),
-          "r"(r[16]), "r"(r[17]), "r"(r[18]), "r"(r[19]), "r"(r[20]), "r"(r[21]), "r"(r[22]), "r"(r[23]),
-          "r"(r[24]), "r"(r[25]), "r"(r[26]), "r"(r[27]), "r"(r[28]), "r"(r[29]), "r"(r[30]), "r"(r[31])
-        : "memory");
-}
-
-#ifdef NMF_TC_TRACE
-// diagnostic timeline (built only with -DNMF_TC_TRACE): (tag, clock64) pairs of CTA 0's third tile
-__device__ long long nmf_tc_trace_buf[3][1024];
-#define TR_DECL int tr_n = 0; int tr_tile = 0;
-#define TR(role, tag) do { if (blockIdx.x == 0 && blockIdx.y == 0 && tr_tile == 2 && lane == 0 && tr_n < 510) { \
-        nmf_tc_trace_buf[role][2 * tr_n] = (tag); nmf_tc_trace_buf[role][2 * tr_n + 1] = clock64(); ++tr_n; } } while (0)
-#define TR_NEXT do { ++tr_tile; } while (0)
-#else
-#define TR_DECL
-#define TR(role, tag) do {} while (0)
-#define TR_NEXT do {} while (0)
-#endif
 
 struct TcArgs {
     CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px]
@@ -289,9 +206,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         const int NSC = (NC + 1) / 2;                    // H-phase super-chunks of 32 frames (the last may hold 16)
         constexpr int NSC2 = NCH2 / 2;                   // W-phase super-chunks of 32 pixels
         uint32_t acc_started = 0;
-        TR_DECL
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
-            TR(0, 1);
             // ---- H phase ----
             auto issue_S = [&](int j) {                  // S(j): [128 px] x [32 frames], K = comps -> Z[j & 1]
                 if (elect_one()) {
@@ -309,17 +224,14 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 __syncwarp();
             };
             wait(B_HS);
-            TR(0, 2);
             if (!proj) {
             issue_S(0);
             if (NSC > 1) issue_S(1);
-            TR(0, 3);
             for (int j = 0; j < NSC; ++j) {
                 for (int gg = 0; gg < 2; ++gg) {
                     const int c = 2 * j + gg;
                     if (c >= NC) break;
                     wait(B_P0 + gg);
-                    TR(0, 100 + c);
                     if (elect_one()) {
                         const uint32_t z = tmem + T_HZ + 32 * (j & 1) + 16 * gg, e = tmem + T_HE + 32 * gg;
                         const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
@@ -339,7 +251,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             }
             if (elect_one()) mma_commit(&bars[B_ND]);
             __syncwarp();
-            TR(0, 4);
             }
             // ---- W phase: one 128-frame M tile at a time; A of S' = the tile's rows of W, staged in TMEM ----
             auto issue_S2 = [&](int j) {                 // S'(j): [128 frames] x [32 px], K = comps -> Z[j & 1]
@@ -357,17 +268,14 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 __syncwarp();
             };
             if (!proj) wait(B_HS2);                      // H' pieces in Hs and W tile 0 in TMEM are in place
-            TR(0, 5);
             for (int m = 0; m < MT; ++m) {
                 if (m > 0) wait(B_WT);                   // W tile m staged (every S' of tile m - 1 has completed)
                 issue_S2(0);
                 issue_S2(1);
-                TR(0, 6);
                 for (int j = 0; j < NSC2; ++j) {
                     for (int gg = 0; gg < 2; ++gg) {
                         const int c = 2 * j + gg;
                         wait(B_P20 + gg);
-                        TR(0, 200 + 10 * m + c);
                         if (elect_one()) {
                             const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
                             const uint32_t z = tmem + T_WZ + 32 * (j & 1) + 16 * gg;
@@ -390,8 +298,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             }
             if (elect_one()) mma_commit(&bars[B_AB]);
             __syncwarp();
-            TR(0, 7);
-            TR_NEXT;
         }
     } else if (warp < EW_WARPS) {
         // =========================== element-wise warps ===========================
@@ -435,16 +341,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         bool first = true;
         const int NSC = (NC + 1) / 2;
         constexpr int NSC2 = NCH2 / 2;
-        TR_DECL
-#ifdef NMF_TC_TRACE
-        const int tr_role = (q == 0) ? 1 + grp : 0;
-#define TRE(tag) do { if (tr_role) TR(tr_role, tag); } while (0)
-#else
-#define TRE(tag) do {} while (0)
-#endif
 
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
-            TRE(1);
             const long long p = tile * TILE + t;
             const bool p_ok = p < P;
             const long long pc = p_ok ? p : P - 1;
@@ -452,7 +350,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             // ---- H0: this group's 32 components of the H tile are split into Hs[pixel][comp] ----
             const float* hsl = nullptr;
             if (grp < KH) hsl = reinterpret_cast<const float*>(wait_full(sq + grp));
-            TRE(2);
             uint32_t hp1[16], hp2[16], hp3[16];
 #pragma unroll
             for (int j = 0; j < 16; ++j) {
@@ -463,7 +360,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             }
             if (!first) { wait(B_AB); }                  // every MMA of the previous tile is complete: Hs is free
             first = false;
-            TRE(3);
 #pragma unroll
             for (int gq = 0; gq < 4; ++gq) {
                 const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + (4 * grp + gq) * HS_SB;
@@ -475,7 +371,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             if (proj) { stage_wt(0); tc_fence_before(); }        // (the previous tile's MMAs are complete: B_AB)
             fence_proxy_async();
             warp_arrive(B_HS);
-            TRE(4);
 
             bool pending = false;                        // an ND / AB of this group may still be reading E[grp]
             if (!proj) {
@@ -487,7 +382,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 if (have) {
                     const uint32_t seq = sq + KH + c;
                     const float* xs = reinterpret_cast<const float*>(wait_full(seq));
-                    TRE(190 + j);
                     const int nv = N - FCH * c;          // valid frames of this chunk (>= 16: all)
 #pragma unroll
                     for (int i = 0; i < 16; ++i) {
@@ -495,9 +389,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         o[i] = i < nv ? xs[FCH * TILE + i * TILE + t] : 0.f;
                     }
                 }
-                TRE(100 + j);
                 wait(B_S0 + (j & 1));                    // both groups track every completion of the buffer's barrier
-                TRE(120 + j);
                 if (have) {
                     tc_fence_after();
                     const uint32_t zcol = lane_base + T_HZ + 32 * (j & 1) + 16 * grp;
@@ -507,25 +399,19 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     ew16(x, o, s, zcol, e);
                     release(sq + KH + c);                // only now: every x, o value has been consumed (a release right
                                                          // after issuing the loads raced with the refill of the slot)
-                    TRE(140 + j);
                     if (pending) { wait(B_NDG0 + grp); tc_fence_after(); }
-                    TRE(160 + j);
                     tmem_st32(lane_base + T_HE + 32 * grp, e);
                     tmem_wait_st();
-                    TRE(170 + j);
                     tc_fence_before();
                     warp_arrive(B_P0 + grp);
-                    TRE(180 + j);
                     pending = true;
                 }
             }
-            TRE(5);
             // ---- UPD: h' = h * num / max(den, eps); thread = (pixel t, this group's 32 comps) ----
             // the old h is rebuilt exactly from its three BF16 pieces in Hs (h = h1 + h2 + h3, every partial sum exact)
             if (pending) wait(B_NDG0 + grp);
             wait(B_ND);                                  // Num, Den complete; every stage-1 read of Hs is done
             tc_fence_after();
-            TRE(6);
             {
                 float* hp = H + (size_t)(32 * grp) * P + pc;
 #pragma unroll
@@ -564,7 +450,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             fence_proxy_async();
             tc_fence_before();
             warp_arrive(B_HS2);
-            TRE(7);
             }   // !proj
 
             // ---- W phase: M tile m, super-chunk j = chunks 2j + grp; thread = (frame 128 m + t, 16 pixels) ----
@@ -580,9 +465,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 for (int j = 0; j < NSC2; ++j) {
                     const int c = 2 * j + grp;
                     const uint32_t seq = sq + KH + NCR + NCH2 * m + c;
-                    TRE(200 + j);
                     const unsigned char* xsl = wait_full(seq);       // X rows at +0, Omega rows at +8 KB
-                    TRE(210 + j);
                     float x[16], o[16];
                     if (active) {
                         if (fr < N) {
@@ -600,7 +483,6 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         }
                     }
                     wait(B_S20 + (j & 1)); tc_fence_after();
-                    TRE(220 + j);
                     uint32_t e[32];
                     if (active) {
                         const uint32_t zcol = lane_base + T_WZ + 32 * (j & 1) + 16 * grp;
@@ -610,20 +492,15 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                         ew16(x, o, s, zcol, e);
                     }
                     release(seq);                        // after the values were consumed (see the H phase)
-                    TRE(230 + j);
                     if (pending) { wait(B_ABG0 + grp); tc_fence_after(); }
-                    TRE(240 + j);
                     if (active) tmem_st32(lane_base + T_WE + 32 * grp, e);
                     tmem_wait_st();
                     tc_fence_before();
                     warp_arrive(B_P20 + grp);
                     pending = true;
-                    TRE(250 + j);
                 }
             }
             wait(B_ABG0 + grp);
-            TRE(8);
-            TR_NEXT;
         }
         wait(B_AB);                                      // every MMA of the last tile is complete
         tc_fence_after();
@@ -659,36 +536,6 @@ constexpr size_t SMEM_MAX = 227 * 1024;
 
 size_t tc_smem_fixed(int NF) { return (size_t)3 * NF * 128 + 3 * HS_BYTES + B_COUNT * 8 + 16; }
 
-// cuTensorMapEncodeTiled through the runtime's driver entry point (no link-time libcuda dependency)
-typedef CUresult (*encode_fn_t)(CUtensorMap*, CUtensorMapDataType, cuuint32_t, void*, const cuuint64_t*, const cuuint64_t*,
-                                const cuuint32_t*, const cuuint32_t*, CUtensorMapInterleave, CUtensorMapSwizzle,
-                                CUtensorMapL2promotion, CUtensorMapFloatOOBfill);
-
-encode_fn_t encode_fn() {
-    static encode_fn_t fn = nullptr;
-    if (!fn) {
-        void* p = nullptr;
-        cudaDriverEntryPointQueryResult qr;
-        if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &p, cudaEnableDefault, &qr) == cudaSuccess &&
-            qr == cudaDriverEntryPointSuccess)
-            fn = reinterpret_cast<encode_fn_t>(p);
-    }
-    return fn;
-}
-
-// 2-D fp32 map over a row-major [rows, P] array, box [box_rows][box_px]
-bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, int box_rows, int box_px, bool swizzle64) {
-    encode_fn_t fn = encode_fn();
-    if (!fn) return false;
-    const cuuint64_t dims[2] = {(cuuint64_t)P, (cuuint64_t)rows};
-    const cuuint64_t strides[1] = {(cuuint64_t)P * sizeof(float)};
-    const cuuint32_t box[2] = {(cuuint32_t)box_px, (cuuint32_t)box_rows};
-    const cuuint32_t estr[2] = {1, 1};
-    return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
-              CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
-}
-
 template <int KS, int PLACE>
 cudaError_t launch_kp(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
     static bool attr_done[64] = {};                      // function attributes are per device
@@ -708,7 +555,7 @@ cudaError_t launch_ks(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, 
 }  // namespace
 
 void nmf_tc_configure(nmf_plan* p) {
-    p->t_ctas = 0; p->t_nst = 0;
+    p->t_ctas = 0;
     if (p->K > KP || p->N > 256) return;
     if (p->P + TILE >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
     const int NF = (p->N + FCH - 1) / FCH * FCH;
@@ -721,7 +568,7 @@ void nmf_tc_configure(nmf_plan* p) {
     if (ctas > n_tiles) ctas = n_tiles;
     const long long per = (n_tiles + ctas - 1) / ctas;      // even out: every CTA gets `per` or one fewer
     ctas = (n_tiles + per - 1) / per;
-    p->t_ctas = (int)ctas; p->t_nst = (int)ns;
+    p->t_ctas = (int)ctas;
 }
 
 size_t nmf_tc_workspace(const nmf_plan* p) {
@@ -733,12 +580,6 @@ size_t nmf_tc_workspace(const nmf_plan* p) {
 }
 
 bool nmf_tc_available(const nmf_plan* p) { return p->t_ctas != 0; }
-
-#ifdef NMF_TC_TRACE
-extern "C" int nmf_debug_tc_trace(long long* host_out) {
-    return (int)cudaMemcpyFromSymbol(host_out, nmf_tc_trace_buf, sizeof(long long) * 3 * 1024);
-}
-#endif
 
 namespace {
 // one launch sequence: `iters` x { fused tile kernel ; fixed-order reduce + update of W (or coef) }

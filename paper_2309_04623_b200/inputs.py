@@ -227,6 +227,13 @@ def make_sweep(K: int, N: int = 200, S: int = 1024, iters: int = 200, M: int = 3
                      name=f"sweep_K{K}")
 
 
+def reinit(lib: Problem, K: int, name: str) -> Problem:
+    """The sweep problem make_sweep(K) built from an already generated STIS-shaped library `lib` (same N, S, M):
+    identical arrays, without regenerating the frames (the library draws do not depend on K)."""
+    W0, H0, C0 = _init_factors(np.random.default_rng(3100 + K), lib.N, K, lib.P, lib.M)
+    return dataclasses.replace(lib, name=name, K=K, W0=W0, H0=H0, C0=C0)
+
+
 def make_survey_problem(b: int, N: int = 128, S: int = 256, K: int = 20, iters: int = 300,
                         M: int = 4) -> Problem:
     """Problem b of the survey batch: MIRI generator, seed 5000+b, occulter radius U[6,14]."""

@@ -13,7 +13,8 @@ from gpu_util import (TOL_FACTOR, check_fit_parity, check_project_subtract_parit
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [1, 2, 0]   # 1 = generic two-kernel path, 2 = fused FFMA, 0 = automatic (tensor-core path when available)
+VARIANTS = [1, 2, 0, 4]   # 1 = generic two-kernel path, 2 = fused FFMA, 0 = automatic (fused tensor-core kernel for K <= 64,
+                          # split tensor-core kernels for K <= 128), 4 = split tensor-core kernels
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
