@@ -20,8 +20,12 @@
  * not multiplied (G5: "treated as missing data and ignored"),
  * and a ratio is num / max(den, 1e-30) (G4).
  *
- * Parity pins for every function here: tests/test_oracle_pins.py (P1-P12).
- * Nothing in this file is "parity unpinned".
+ * Parity pins for every function here: tests/test_oracle_pins.py (P1-P24).
+ * "Parity unpinned": only the CONVENTIONS of oracle_derotate_stack (rotation centre,
+ * bilinear interpolation, mean combination: readings G22-G24 -- the paper states none,
+ * PAPER.md:89, 99); the arithmetic those readings define is pinned (P20-P23).  The
+ * stopping quantity of oracle_fit_tol is likewise a reading (G21; PAPER.md:53 names no
+ * quantity); the function is pinned to that reading (P17-P19).
  *
  * Build: gcc -O2 -fopenmp -fPIC -shared -o liboracle.so nmf_oracle.c -lm
  */
@@ -212,4 +216,112 @@ void oracle_ref_select(int M, int N, const double* D, int n_sel, int* idx /* [M,
             if (rank < n_sel) idx[(size_t)m * n_sel + rank] = n;
         }
     }
+}
+
+/* ---- tolerance-based stopping ---------------------------------- */
+/* the iteration is "left to continue until the change in gradient from one
+ * step to the next reaches a set value or the maximum number of iterations is reached".
+ * Neither the quantity nor the value is defined in the paper.  Reading G21:
+ * the monitored quantity is the cost of Eq. 2, f_t, evaluated after every
+ * `check_every` iterations (check_every = 1: "from one step to the next"); the fit stops
+ * at the first check t with  |f_{t-check_every} - f_t| < tol * f_{t-check_every}
+ * (relative change of the cost between consecutive checks, strict inequality: tol = 0
+ * never stops and gives the fixed-count fit), else after max_iters iterations.
+ * Returns the number of iterations done; *f_last = cost at the last check (or f_0);
+ * trace (nullable) receives f_0 and the cost at every check.
+ * Pins: tests/test_oracle_pins.py P17-P19.                                               */
+int oracle_fit_tol(int N, long P, int K, const float* X, const float* Om, double* W, double* H,
+                   int max_iters, int check_every, double tol, double* f_last, double* trace) {
+    double f_prev = oracle_objective(N, P, K, X, Om, W, H);
+    int it = 0;
+    if (trace) trace[0] = f_prev;
+    while (it < max_iters) {
+        oracle_h_step(N, P, K, X, Om, W, H);
+        oracle_w_step(N, P, K, X, Om, W, H);
+        ++it;
+        if (it % check_every == 0) {
+            const double f = oracle_objective(N, P, K, X, Om, W, H);
+            const int stop = fabs(f_prev - f) < tol * f_prev;
+            if (trace) trace[it / check_every] = f;
+            f_prev = f;
+            if (stop) break;
+        }
+    }
+    if (f_last) *f_last = f_prev;
+    return it;
+}
+
+/* ---- derotate + stack ------------------------------------------- */
+/* the PSF-subtracted images "are rotated North-up using their position angles
+ * ... then combined"; PAPER.md:99 likewise for MIRI.  The paper delegates both steps to
+ * third-party tools and states no convention.  Readings (G22-G25):
+ *  G22  frames are ny x nx images, pixel (y, x) at index y*nx + x, rotation centre at the
+ *       pixel (cy, cx) = (ny/2, nx/2) (integer division; the generators' star position).
+ *       Frame m is rotated by angle[m] degrees, counter-clockwise with x to the right and
+ *       y (row index) up: output pixel (y, x) takes the input at
+ *         xs = cx + c*(x-cx) + s*(y-cy),   ys = cy - s*(x-cx) + c*(y-cy),  (s, c) = sin, cos(angle),
+ *       evaluated in fp64 with quadrant-exact sine/cosine (multiples of 90 degrees move
+ *       pixels exactly).  The caller supplies the rotation to apply (the sign that takes a
+ *       position angle to North-up is an instrument convention the paper does not state).
+ *  G23  bilinear interpolation over the four neighbours (y0, x0) .. (y0+1, x0+1),
+ *       (x0, y0) = floor(xs, ys).  Neighbours with weight <= 1e-6 are ignored.  The
+ *       sample is valid only if every remaining neighbour lies inside the image and
+ *       (when a weight/mask frame is given) has omega > 0; otherwise frame m contributes
+ *       nothing at this pixel ("missing data").  Weights are not renormalised.
+ *  G24  combination = mean over the frames with a valid sample (the paper says only
+ *       "combined"); a pixel with no valid sample gets `fill`.  count (nullable) receives
+ *       the number of frames averaged.
+ * Pins: tests/test_oracle_pins.py P20-P24.  Only the interpolation / combination
+ * conventions above are "parity unpinned" against the paper (it states none); the
+ * arithmetic they define is pinned.                                                         */
+static void sincos_deg(double deg, double* s, double* c) {
+    double a = fmod(deg, 360.0);
+    if (a < 0.0) a += 360.0;
+    const int k = (int)floor(a / 90.0 + 0.5);            /* nearest multiple of 90: 0..4 */
+    const double r = (a - 90.0 * k) * (3.14159265358979323846 / 180.0);
+    const double sr = sin(r), cr = cos(r);               /* |r| <= 45 degrees; r = 0 gives exactly (0, 1) */
+    switch (k & 3) {
+        case 0: *s = sr;  *c = cr;  break;
+        case 1: *s = cr;  *c = -sr; break;
+        case 2: *s = -sr; *c = -cr; break;
+        default: *s = -cr; *c = sr; break;
+    }
+}
+
+void oracle_derotate_stack(int M, int ny, int nx, const float* R /* [M, ny*nx] */,
+                           const float* om /* [M, ny*nx] nullable */, const double* angle_deg /* [M] */,
+                           double fill, double* out /* [ny*nx] */, int* count /* [ny*nx] nullable */) {
+    const long P = (long)ny * nx;
+    const int cy = ny / 2, cx = nx / 2;
+    double* sn = (double*)malloc(sizeof(double) * M);
+    double* cs = (double*)malloc(sizeof(double) * M);
+    for (int m = 0; m < M; ++m) sincos_deg(angle_deg[m], &sn[m], &cs[m]);
+#pragma omp parallel for schedule(static)
+    for (int y = 0; y < ny; ++y)
+        for (int x = 0; x < nx; ++x) {
+            const double dx = x - cx, dy = y - cy;
+            double sum = 0.0;
+            int cnt = 0;
+            for (int m = 0; m < M; ++m) {
+                const double xs = cx + cs[m] * dx + sn[m] * dy;
+                const double ys = cy - sn[m] * dx + cs[m] * dy;
+                const double x0 = floor(xs), y0 = floor(ys);
+                const double fx = xs - x0, fy = ys - y0;
+                const double w[4] = {(1.0 - fx) * (1.0 - fy), fx * (1.0 - fy), (1.0 - fx) * fy, fx * fy};
+                int valid = 1;
+                double v = 0.0;
+                for (int i = 0; i < 4; ++i) {
+                    if (!(w[i] > 1e-6)) continue;
+                    const double xi = x0 + (i & 1), yi = y0 + (i >> 1);
+                    if (xi < 0 || xi >= nx || yi < 0 || yi >= ny) { valid = 0; break; }
+                    const size_t j = (size_t)m * P + (size_t)yi * nx + (size_t)xi;
+                    if (om && !((double)om[j] > 0.0)) { valid = 0; break; }
+                    v += w[i] * (double)R[j];
+                }
+                if (valid) { sum += v; ++cnt; }
+            }
+            out[(size_t)y * nx + x] = cnt ? sum / cnt : fill;
+            if (count) count[(size_t)y * nx + x] = cnt;
+        }
+    free(sn); free(cs);
 }

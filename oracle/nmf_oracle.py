@@ -47,6 +47,11 @@ def _load():
                                        ctypes.c_int]
         lib.oracle_subtract.argtypes = [ctypes.c_int, ctypes.c_long, ctypes.c_int, _D, _F, _D, _F,
                                         _D, ctypes.c_double, _D]
+        lib.oracle_fit_tol.restype = ctypes.c_int
+        lib.oracle_fit_tol.argtypes = [ctypes.c_int, ctypes.c_long, ctypes.c_int, _F, _F, _D, _D,
+                                       ctypes.c_int, ctypes.c_int, ctypes.c_double, _D, _D]
+        lib.oracle_derotate_stack.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_int, _F, _F, _D,
+                                              ctypes.c_double, _D, ctypes.POINTER(ctypes.c_int)]
         lib.oracle_ref_distance.argtypes = [ctypes.c_int, ctypes.c_int, ctypes.c_long, _F, _F, _F, _F, _D]
         lib.oracle_ref_select.argtypes = [ctypes.c_int, ctypes.c_int, _D, ctypes.c_int, ctypes.POINTER(ctypes.c_int)]
         _lib = lib
@@ -101,6 +106,36 @@ def fit(X, Omega, W0, H0, iters: int, trace: bool = False):
     tp = tr.ctypes.data_as(_D) if trace else None
     _load().oracle_fit(N, P, K, xp, op, wp, hp, int(iters), tp)
     return (W, H, tr) if trace else (W, H)
+
+
+def fit_tol(X, Omega, W0, H0, max_iters: int, check_every: int, tol: float):
+    """Fit with the tolerance stop of reading G21.  Returns (W, H, iters_done, f_last, trace)
+    with trace = [f_0, cost at every check made]."""
+    X, xp = _f32(X); Om, op = _f32(Omega); W, wp = _f64(W0, copy=True); H, hp = _f64(H0, copy=True)
+    N, P = X.shape; K = W.shape[1]
+    assert Om.shape == (N, P) and W.shape == (N, K) and H.shape == (K, P) and check_every >= 1
+    tr = np.full(max_iters // check_every + 1, np.nan)
+    fl = ctypes.c_double(0.0)
+    it = _load().oracle_fit_tol(N, P, K, xp, op, wp, hp, int(max_iters), int(check_every), float(tol),
+                                ctypes.byref(fl), tr.ctypes.data_as(_D))
+    return W, H, int(it), fl.value, tr[:it // check_every + 1]
+
+
+def derotate_stack(R, omega, angles_deg, ny: int, nx: int, fill: float = 0.0):
+    """Rotate the M frames R [M, ny*nx] by angles_deg (readings G22-G23) and average the valid samples (G24).
+    Returns (stack [ny*nx] fp64, count [ny*nx] int32)."""
+    R, rp = _f32(R)
+    M, P = R.shape
+    assert P == ny * nx
+    op = None
+    if omega is not None:
+        om, op = _f32(omega)
+    ang, ap = _f64(angles_deg)
+    out = np.empty(P, dtype=np.float64)
+    cnt = np.empty(P, dtype=np.int32)
+    _load().oracle_derotate_stack(M, int(ny), int(nx), rp, op, ap, float(fill), out.ctypes.data_as(_D),
+                                  cnt.ctypes.data_as(ctypes.POINTER(ctypes.c_int)))
+    return out, cnt
 
 
 def project(H, T, omega_t, C0, iters: int):

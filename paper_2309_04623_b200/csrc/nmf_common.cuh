@@ -7,6 +7,7 @@
 #include <string>
 #include "../../include/nmf.h"
 
+#define NMF_MAX_DEVICES 64   // plan->device is checked against this at plan creation
 #define NMF_EPS 1e-30f   // ratio guard: num / max(den, NMF_EPS)   (reading G4)
 
 // ---------------------------------------------------------------------------

@@ -287,9 +287,15 @@ inline GenericCfg pick_cfg(int K) {
 
 constexpr int W_NF = 2;   // frames per thread in the W half-step
 
+constexpr size_t GW_SMEM_MAX = 160 * 1024;   // opt-in dynamic shared memory of k_w_partial
+
 inline void w_geometry(int rows, int kc, int ks, int* nfb, int* NBc, int* threads) {
-    // NBc frames per CTA, (NBc / NF) * KS threads, at most 512 (256 for KC = 16) threads
-    const int nb_max = (kc > 13 ? 256 : 512) / ks * W_NF;
+    // NBc frames per CTA, (NBc / NF) * KS threads, at most 512 (256 for KC = 16) threads, and the staged X / Omega
+    // rows (2 NBc rows of GW_XS floats beside the H' chunk) must fit the opt-in shared memory: with ks = 1 the
+    // thread limit alone allows 1024 frames per CTA = 288 KB (projection of many frames at K <= 13)
+    int nb_max = (kc > 13 ? 256 : 512) / ks * W_NF;
+    const int nb_smem = (int)((GW_SMEM_MAX / sizeof(float) - (size_t)GW_TP * ks * round4(kc)) / (2 * GW_XS)) / W_NF * W_NF;
+    if (nb_max > nb_smem) nb_max = nb_smem;
     *nfb = (rows + nb_max - 1) / nb_max;
     int per = (rows + *nfb - 1) / *nfb;
     per = (per + W_NF - 1) / W_NF * W_NF;
@@ -307,10 +313,10 @@ int launch_h(nmf_plan* p, const float* X, const float* Om, const float* W, float
     const long long pairs_per_cta = GH_THREADS / KS;
     dim3 grid((unsigned)((p->P / 2 + pairs_per_cta - 1) / pairs_per_cta), batch);
     size_t smem = sizeof(float) * (size_t)p->N * KS * round4(KC);
-    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
-    if (!attr_done) {
+    static bool attr_done[NMF_MAX_DEVICES] = {};   // function attributes are per device
+    if (!attr_done[p->device]) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_h_step<KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
+        attr_done[p->device] = true;
     }
     k_h_step<KC><<<grid, GH_THREADS, smem, p->stream>>>(X, Om, W, H, p->N, p->P, p->K, KS);
     p->launches++;
@@ -324,11 +330,12 @@ int launch_w(nmf_plan* p, const float* X, const float* Om, float* W, const float
     int nfb, NBc, threads;
     w_geometry(rows, KC, KS, &nfb, &NBc, &threads);
     size_t smem = w_smem(KC, KS, NBc);
-    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
-    if (!attr_done) {
-        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_w_partial<KC, W_NF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_w_partial<KC, W_NF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, 160 * 1024));
-        attr_done = true;
+    if (smem > GW_SMEM_MAX) return NMF_ERR_UNSUPPORTED;       // (w_geometry caps NBc so that this cannot happen)
+    static bool attr_done[NMF_MAX_DEVICES] = {};   // function attributes are per device
+    if (!attr_done[p->device]) {
+        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_w_partial<KC, W_NF, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GW_SMEM_MAX));
+        NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_w_partial<KC, W_NF, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GW_SMEM_MAX));
+        attr_done[p->device] = true;
     }
     dim3 grid(parts, nfb, batch);
     float* slab = reinterpret_cast<float*>(p->ws);
@@ -336,9 +343,11 @@ int launch_w(nmf_plan* p, const float* X, const float* Om, float* W, const float
         k_w_partial<KC, W_NF, true><<<grid, threads, smem, p->stream>>>(X, Om, W, H, slab, rows, p->P, p->K, KS, NBc);
     else
         k_w_partial<KC, W_NF, false><<<grid, threads, smem, p->stream>>>(X, Om, W, H, slab, rows, p->P, p->K, KS, NBc);
+    NMF_CUDA_TRY(p, cudaGetLastError());           // a failed launch must not let the update read an unwritten slab
+    p->launches++;
     dim3 g2((rows * p->K + WU_E - 1) / WU_E, batch);
     k_w_update<<<g2, WU_E * WU_Q, 0, p->stream>>>(slab, W, rows, p->K, KC * KS, parts);
-    p->launches += 2;
+    p->launches++;
     return NMF_OK;
 }
 

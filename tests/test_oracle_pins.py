@@ -364,3 +364,184 @@ def test_p16_ref_select_order_and_ties():
     X[5] = T[0]; X[1] = T[2]
     idx = orc.ref_select(orc.ref_distance(T, ot, X, Om), 4)
     assert idx[0, 0] == 5 and idx[2, 0] == 1
+
+
+# ---- P17-P19: tolerance-based stopping (reading G21) -------------------------
+def test_p17_fit_tol_worked_example():
+    """The stop index on the exact-rational example follows from the golden costs (f_0 = 46,
+    f after iteration 1 = 16.32935302, after iteration 2 = 15.70666801): the relative changes are 0.6450 and
+    0.03813, so tol = 0.04 stops after iteration 2, tol = 0.038 does not, tol = 0.7 stops after iteration 1."""
+    g = _load_p4()
+    X, Om, W0, H0 = g["X"], g["Omega"], g["W0"], g["H0"]
+    f0, f1, f2 = 46.0, g["f_W1"][0, 0], g["f_W2"][0, 0]
+    assert (f0 - f1) / f0 == pytest.approx(0.64501, abs=1e-4) and (f1 - f2) / f1 == pytest.approx(0.038133, abs=1e-5)
+    W, H, it, fl, tr = orc.fit_tol(X, Om, W0, H0, 10, 1, 0.7)
+    assert it == 1 and fl == pytest.approx(f1, rel=2e-9)
+    W, H, it, fl, tr = orc.fit_tol(X, Om, W0, H0, 10, 1, 0.04)
+    assert it == 2 and fl == pytest.approx(f2, rel=2e-9)
+    np.testing.assert_allclose(W, g["W2"], rtol=2e-9); np.testing.assert_allclose(H, g["H2"], rtol=2e-9, atol=0)
+    np.testing.assert_allclose(tr, [f0, f1, f2], rtol=2e-9)
+    W, H, it, fl, tr = orc.fit_tol(X, Om, W0, H0, 2, 1, 0.038)
+    assert it == 2                                        # max_iters reached, not the tolerance
+    W, H, it, fl, tr = orc.fit_tol(X, Om, W0, H0, 3, 1, 0.038)
+    assert it == 3
+    # check_every = 2: the only check in 2 iterations compares f_0 with f after iteration 2 (change 0.6586 < 0.7)
+    W, H, it, fl, tr = orc.fit_tol(X, Om, W0, H0, 10, 2, 0.7)
+    assert it == 2 and (f0 - f2) / f0 == pytest.approx(0.65855, abs=1e-4)
+    np.testing.assert_allclose(tr, [f0, f2], rtol=2e-9)
+
+
+def test_p18_fit_tol_equals_trace_scan(tiny):
+    """The early exit stops exactly where a scan of the fixed-count fit's cost trace says, with the iterates of
+    that many fixed-count iterations (bitwise), for several tolerances and check intervals; tol = 0 never stops."""
+    p = tiny
+    _, _, tr = orc.fit(p.X, p.Omega, p.W0, p.H0, 120, trace=True)
+    f = tr[0::2]                                          # cost after every full iteration (tr holds both half-steps)
+    last = 120
+    for m in (1, 4, 7):
+        for tol in (0.0, 1e-4, 1e-3, 1e-2, 0.3):
+            checks = np.arange(m, 121, m)
+            hit = [t for t in checks if abs(f[t - m] - f[t]) < tol * f[t - m]]
+            expect = hit[0] if hit else 120
+            W, H, it, fl, trc = orc.fit_tol(p.X, p.Omega, p.W0, p.H0, 120, m, tol)
+            assert it == expect, (m, tol, it, expect)
+            Wf, Hf = orc.fit(p.X, p.Omega, p.W0, p.H0, it)
+            assert np.array_equal(W, Wf) and np.array_equal(H, Hf)
+            assert fl == f[it // m * m] and np.array_equal(trc, f[0:it // m * m + 1:m])
+            if tol == 0.0:
+                assert it == 120
+        # P1: the cost is non-increasing, so a looser tolerance can only stop earlier
+        its = [orc.fit_tol(p.X, p.Omega, p.W0, p.H0, 120, m, tol)[2] for tol in (1e-5, 1e-4, 1e-3, 1e-2, 1e-1)]
+        assert all(a >= b for a, b in zip(its, its[1:])), its
+        assert its[0] <= last
+
+
+def test_p19_fit_tol_fixed_point_never_stops_at_zero_cost():
+    """X = W*H* exactly with the fit started at (W*, H*): every cost is 0 and the strict test |df| < tol * f never
+    fires -- the fit runs to max_iters (a non-strict test would stop at once; G21 fixes the strict form)."""
+    rng = np.random.default_rng(5)
+    Ws = rng.integers(1, 4, (5, 2)).astype(np.float64); Hs = rng.integers(1, 4, (2, 24)).astype(np.float64)
+    X = (Ws @ Hs).astype(np.float32); Om = np.ones_like(X)
+    W, H, it, fl, tr = orc.fit_tol(X, Om, Ws, Hs, 9, 1, 0.5)
+    assert it == 9 and fl == 0.0
+
+
+# ---- P20-P24: derotate + stack (SURVEY.md 8(f) NEXT-4; PAPER.md:89, 99; readings G22-G24) -------------------------
+def _frames(M, ny, nx, seed):
+    rng = np.random.default_rng(seed)
+    return (rng.random((M, ny * nx)) * 10 - 3).astype(np.float32)
+
+
+def test_p20_derotate_quarter_turns_are_exact_pixel_moves():
+    """Multiples of 90 degrees move pixels exactly.  With an odd side the centre pixel (n/2, n/2) is the array
+    centre, so a counter-clockwise quarter turn (x right, y = row index up) is numpy's rot90 with k = -1 seen in
+    row-down display, i.e. out[y, x] = in[cy - (x - cx), cx + (y - cy)]: compared with the library routine."""
+    n = 9
+    R = _frames(1, n, n, 1)
+    img = R[0].reshape(n, n)
+    out0, cnt = orc.derotate_stack(R, None, [0.0], n, n)
+    assert np.array_equal(out0.reshape(n, n), img.astype(np.float64)) and np.all(cnt == 1)
+    out360, _ = orc.derotate_stack(R, None, [360.0], n, n)
+    assert np.array_equal(out360, out0)
+    out90, cnt = orc.derotate_stack(R, None, [90.0], n, n)
+    # reading G22 at 90 degrees: source (xs, ys) = (cx + dy, cy - dx)
+    ref = np.empty((n, n))
+    c = n // 2
+    for y in range(n):
+        for x in range(n):
+            ref[y, x] = img[c - (x - c), c + (y - c)]
+    assert np.array_equal(out90.reshape(n, n), ref) and np.all(cnt == 1)
+    assert np.array_equal(ref, np.rot90(img, k=-1).astype(np.float64))     # library routine (rows stored top-down: k = -1)
+    out180, _ = orc.derotate_stack(R, None, [180.0], n, n)
+    assert np.array_equal(out180.reshape(n, n), img[::-1, ::-1].astype(np.float64))
+    out270, _ = orc.derotate_stack(R, None, [-90.0], n, n)
+    assert np.array_equal(out270.reshape(n, n), np.rot90(img, k=1).astype(np.float64))
+    # four quarter turns compose to the identity
+    a = R
+    for _ in range(4):
+        o, _ = orc.derotate_stack(a, None, [90.0], n, n)
+        a = o.astype(np.float32)[None, :]
+    assert np.array_equal(a, R)
+
+
+def test_p20b_even_side_centre_convention():
+    """Even side: the centre is the pixel (n/2, n/2), not the array centre, so a half turn maps pixel i to n - i:
+    row / column 0 has no source inside the image and is filled."""
+    n = 8
+    R = _frames(1, n, n, 2)
+    img = R[0].reshape(n, n).astype(np.float64)
+    out, cnt = orc.derotate_stack(R, None, [180.0], n, n, fill=-7.0)
+    o = out.reshape(n, n); cn = cnt.reshape(n, n)
+    assert np.all(o[0, :] == -7.0) and np.all(o[:, 0] == -7.0) and np.all(cn[0, :] == 0) and np.all(cn[1:, 1:] == 1)
+    assert np.array_equal(o[1:, 1:], img[1:, 1:][::-1, ::-1])
+
+
+def test_p21_derotate_matches_library_bilinear():
+    """Generic angles against scipy.ndimage.map_coordinates(order=1) evaluated at the source coordinates of G22
+    (library bilinear interpolation); pixels whose neighbours leave the image are excluded by both."""
+    from scipy import ndimage
+    ny, nx = 21, 26
+    R = _frames(3, ny, nx, 3)
+    cy, cx = ny // 2, nx // 2
+    yy, xx = np.mgrid[0:ny, 0:nx].astype(np.float64)
+    for ang in (17.0, -41.5, 133.0):
+        s, c = np.sin(np.deg2rad(ang)), np.cos(np.deg2rad(ang))
+        xs = cx + c * (xx - cx) + s * (yy - cy)
+        ys = cy - s * (xx - cx) + c * (yy - cy)
+        inside = (xs >= 0) & (xs <= nx - 1) & (ys >= 0) & (ys <= ny - 1)
+        for m in range(3):
+            ref = ndimage.map_coordinates(R[m].reshape(ny, nx).astype(np.float64), [ys, xs], order=1, mode="nearest")
+            out, cnt = orc.derotate_stack(R[m:m + 1], None, [ang], ny, nx, fill=np.nan)
+            o = out.reshape(ny, nx); cn = cnt.reshape(ny, nx)
+            strict = (xs >= 0) & (xs < nx - 1) & (ys >= 0) & (ys < ny - 1)
+            assert np.all(cn[strict] == 1) and np.all(cn[~inside] == 0)
+            np.testing.assert_allclose(o[strict], ref[strict], rtol=0, atol=1e-12)
+
+
+def test_p22_derotate_constant_linearity_and_mean():
+    ny, nx, M = 17, 19, 5
+    rng = np.random.default_rng(4)
+    ang = rng.uniform(-180, 180, M)
+    # a constant image stays constant wherever a sample exists (bilinear weights sum to 1)
+    Cst = np.full((M, ny * nx), 2.5, dtype=np.float32)
+    out, cnt = orc.derotate_stack(Cst, None, ang, ny, nx, fill=np.nan)
+    assert np.all(np.abs(out[cnt > 0] - 2.5) < 1e-5)              # (ignored neighbours carry weight <= 1e-6 each)
+    assert np.all(np.isnan(out[cnt == 0]))
+    # linear in the frames
+    A, B = np.round(_frames(M, ny, nx, 5) * 8), np.round(_frames(M, ny, nx, 6) * 8)     # small integers: 2A - 3B is exact in fp32
+    oa, ca = orc.derotate_stack(A, None, ang, ny, nx)
+    ob, _ = orc.derotate_stack(B, None, ang, ny, nx)
+    oab, _ = orc.derotate_stack((2 * A - 3 * B).astype(np.float32), None, ang, ny, nx)
+    lin = 2 * A.astype(np.float64) - 3 * B.astype(np.float64)
+    assert np.array_equal(lin.astype(np.float32).astype(np.float64), lin)   # exactly representable inputs
+    np.testing.assert_allclose(oab, 2 * oa - 3 * ob, rtol=0, atol=1e-10)
+    # identical frames at angle 0 average to themselves; the stack is the mean of the single-frame results
+    one = _frames(1, ny, nx, 7)
+    rep, cnt = orc.derotate_stack(np.repeat(one, 4, axis=0), None, [0, 0, 0, 0], ny, nx)
+    assert np.array_equal(rep, one[0].astype(np.float64)) and np.all(cnt == 4)
+    singles = [orc.derotate_stack(A[m:m + 1], None, ang[m:m + 1], ny, nx) for m in range(M)]
+    num = sum(o * (c > 0) for o, c in singles); den = sum((c > 0).astype(int) for o, c in singles)
+    np.testing.assert_allclose(oa[den > 0], num[den > 0] / den[den > 0], rtol=0, atol=1e-12)
+    assert np.array_equal(ca, den)
+
+
+def test_p23_derotate_mask_semantics():
+    """A masked source pixel (omega == 0) invalidates exactly the output samples that touch it with weight > 1e-6;
+    its value (NaN / Inf) never enters the result."""
+    ny, nx = 15, 15
+    R = _frames(2, ny, nx, 8)
+    om = np.ones_like(R)
+    om[0, 7 * nx + 4] = 0.0; om[1, 3 * nx + 9] = 0.0
+    Rg = R.copy(); Rg[om == 0] = np.nan
+    ang = [30.0, 0.0]
+    o1, c1 = orc.derotate_stack(R, om, ang, ny, nx, fill=0.0)
+    o2, c2 = orc.derotate_stack(Rg, om, ang, ny, nx, fill=0.0)
+    assert np.array_equal(o1, o2) and np.array_equal(c1, c2) and np.all(np.isfinite(o2))
+    # frame 1 (angle 0): only its own pixel loses a sample
+    full, cfull = orc.derotate_stack(R, None, ang, ny, nx)
+    lost = (cfull - c1).reshape(ny, nx)
+    assert lost[3, 9] >= 1 and lost.sum() <= 1 + 4          # frame 0's masked pixel touches at most 4 outputs
+    # every frame masked at a pixel -> fill
+    om[:, :] = 0.0
+    o3, c3 = orc.derotate_stack(R, om, ang, ny, nx, fill=-1.0)
+    assert np.all(o3 == -1.0) and np.all(c3 == 0)
