@@ -36,6 +36,15 @@
  *     Omega > 0; Omega >= 0; W, H, coef >= 0 on entry (an exact zero stays zero).
  *   - Results are bitwise reproducible run to run for a fixed plan shape on a
  *     fixed device (all cross-CTA sums are fixed-order).
+ *   - Arithmetic.  Inputs and results are fp32.  The default (tensor-core) kernel
+ *     families evaluate the six contractions of Eq. 3 with every fp32 operand split
+ *     exactly into three BF16 pieces and six piece products per product, accumulated
+ *     in fp32 (dropped terms <= 2^-22 relative, the level of a 3xTF32 split); the
+ *     H update divides with the fast reciprocal (<= 2 ulp); sums across CTAs are
+ *     fp64 in a fixed order.  The FFMA families (variants 1, 2) use plain fp32 FMA.
+ *     Families therefore agree to fp32 rounding level, not bitwise.
+ *   - A plan is bound to the CUDA device that was current when it was created;
+ *     every call must be made with that device current (else INVALID_ARG).
  */
 #ifndef PAPER_2309_04623_NMF_H
 #define PAPER_2309_04623_NMF_H
@@ -50,7 +59,8 @@ typedef enum nmf_status {
     NMF_OK = 0,
     NMF_ERR_INVALID_ARG = -1, /* null pointer; N/P/K/M/iters out of range; M > max_targets   */
     NMF_ERR_ALIGNMENT   = -2, /* base pointer not 16-byte aligned or P % 4 != 0              */
-    NMF_ERR_UNSUPPORTED = -3, /* N > 256 or K > 128 (compiled limits)                        */
+    NMF_ERR_UNSUPPORTED = -3, /* N > 256, K > 128 or max_targets > 4096 (compiled limits); a
+                                 forced variant (2, 3, 4) whose kernels do not cover the shape */
     NMF_ERR_WORKSPACE   = -4, /* workspace missing or smaller than nmf_plan_workspace_bytes  */
     NMF_ERR_ARCH        = -5, /* current device is not compute capability 10.x               */
     NMF_ERR_CUDA        = -6  /* CUDA runtime / launch error (sticky until the plan is freed) */
@@ -78,12 +88,20 @@ int nmf_plan_set_workspace(nmf_plan* plan, void* workspace_dev, size_t bytes);
 /* cudaStream_t to enqueue on, passed as void*.  NULL = the legacy default stream. */
 int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
 
-/* Select the fit kernel family: 0 = automatic (fused per-pixel-tile kernel when
- * the shape is inside its compiled range, else the generic two-kernel path),
- * 1 = force generic, 2 = force fused (UNSUPPORTED at fit time if out of range).
- * Both families compute the same updates; they differ in summation order only.  */
+/* Select the kernel family of nmf_fit / nmf_fit_batched / nmf_project:
+ *   0  automatic: the fastest family that covers the shape (a tensor-core family
+ *      whenever K <= 128 and the operands fit shared memory, else FFMA)
+ *   1  generic two-kernel FFMA path (any N <= 256, K <= 128; also what
+ *      nmf_project runs when omega == NULL)
+ *   2  fused FFMA per-pixel-tile kernel (K <= 50)
+ *   3  fused tcgen05 kernel: one kernel per iteration does both half-steps (K <= 64)
+ *   4  split tcgen05 kernels: H half-step kernel + W half-step kernel (K <= 128;
+ *      N = 256 only up to K = 96)
+ * A forced family (2, 3, 4) that does not cover the plan's shape makes the fit
+ * return UNSUPPORTED.  All families compute the updates of Eq. 3; see "Arithmetic"
+ * above for how they differ.  Errors: INVALID_ARG (variant outside 0..4).          */
 int nmf_plan_set_variant(nmf_plan* plan, int variant);
-/* Which family nmf_fit will run for this plan: 1 = generic, 2 = fused.            */
+/* Which family (1..4) nmf_fit will run for this plan.                              */
 int nmf_plan_get_variant(const nmf_plan* plan);
 
 int nmf_plan_destroy(nmf_plan* plan); /* frees host state and any internal staging buffers */
@@ -103,7 +121,8 @@ int nmf_fit_batched(nmf_plan* plan, const float* X, const float* Omega, float* W
 
 /* Target modelling: non-negative projection of M science frames on fixed H by
  * `iters` W-type updates of Eq. 3, c <- c o (omega o t)H^T / (omega o (cH))H^T,
- * each frame independently.
+ * each frame independently.  Runs the plan's tensor-core family when
+ * omega is given, the generic FFMA path when omega == NULL.
  *   H       device [K,P]  read-only     target device [M,P] read-only
  *   omega   device [M,P]  read-only, or NULL = all ones
  *   coef    device [M,K]  in: initial coefficients, out: result (in place)
@@ -119,8 +138,24 @@ int nmf_project(nmf_plan* plan, const float* H, const float* target, const float
 int nmf_subtract(nmf_plan* plan, const float* H, const float* target, const float* coef,
                  const float* omega, const float* factor, float fill, float* out, int M);
 
-/* Diagnostic: the cost of Eq. 2, sum over Omega>0 of
- * Omega*(X-WH)^2, accumulated in fp64.  SYNCHRONISES the plan's stream and
+/* Component construction with the paper's stopping rule ("until the
+ * change in gradient from one step to the next reaches a set value or the maximum
+ * number of iterations is reached"; the quantity is not defined there -- reading
+ * G21 in DESIGN.md): the cost f of Eq. 2 is evaluated on the device (fp64, fixed
+ * order) at the start and after every `check_every` iterations, and the fit stops
+ * at the first check t with |f_(t-check_every) - f_t| < tol * f_(t-check_every),
+ * else after max_iters iterations.  tol = 0 never stops early (= nmf_fit).
+ *   X, Omega, W, H  device, as for nmf_fit (single problem)
+ *   iters_done      host, out: iterations performed
+ *   f_last          host, out, nullable: cost at the last check (f_0 if none made)
+ * SYNCHRONISES once per check (every `check_every` iterations), not per iteration.
+ * Errors: INVALID_ARG (check_every < 1, tol < 0 or NaN, ...), ALIGNMENT, WORKSPACE,
+ * CUDA.                                                                            */
+int nmf_fit_tol(nmf_plan* plan, const float* X, const float* Omega, float* W, float* H,
+                int max_iters, int check_every, double tol, int* iters_done, double* f_last);
+
+/* The cost of Eq. 2, sum over Omega>0 of Omega*(X-WH)^2, accumulated
+ * in fp64 on the device in a fixed order.  SYNCHRONISES the plan's stream and
  * writes one double to host memory.                                               */
 int nmf_objective(nmf_plan* plan, const float* X, const float* Omega, const float* W,
                   const float* H, double* out_host);
@@ -163,6 +198,26 @@ int nmf_ref_distance(nmf_plan* plan, const float* target, const float* omega_t, 
  *   dist device [M,N] read-only     idx device [M,n_sel] out (int32)
  * Errors: INVALID_ARG, CUDA.                                                       */
 int nmf_ref_select(nmf_plan* plan, const float* dist, int M, int n_sel, int* idx);
+
+/* Derotate + stack (the subtracted frames "are rotated North-up
+ * using their position angles ... then combined"; the paper states no convention:
+ * readings G22-G24 in DESIGN.md).  Frame m (an ny x nx image, pixel (y, x) at
+ * y*nx + x, ny*nx == the plan's P) is rotated by angle_deg[m] degrees, counter-
+ * clockwise with x to the right and y up, about the pixel (ny/2, nx/2): output
+ * pixel (y, x) samples the input at
+ *   xs = cx + cos(a)(x-cx) + sin(a)(y-cy),  ys = cy - sin(a)(x-cx) + cos(a)(y-cy)
+ * by bilinear interpolation (fp64 coordinates, exact at multiples of 90 degrees;
+ * neighbours with weight <= 1e-6 ignored).  A sample counts only if all its
+ * neighbours are inside the image and have omega > 0 (masked pixels may hold
+ * NaN/Inf).  out = mean over the frames with a sample, `fill` where
+ * there is none; count (nullable) = number of frames averaged.
+ *   resid device [M,P] read-only      omega device [M,P] or NULL = all valid
+ *   angle_deg device [M] fp32         out device [P]   count device [P] int32 or NULL
+ * M is not limited by max_targets.  Errors: INVALID_ARG (ny*nx != P, ...),
+ * ALIGNMENT, CUDA.                                                                 */
+int nmf_derotate_stack(nmf_plan* plan, const float* resid, const float* omega,
+                       const float* angle_deg, int ny, int nx, float fill, float* out,
+                       int* count, int M);
 
 /* Number of kernel launches this plan has enqueued so far (bench bookkeeping).     */
 long long nmf_plan_launch_count(const nmf_plan* plan);

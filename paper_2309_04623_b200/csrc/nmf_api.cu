@@ -21,7 +21,16 @@ size_t plan_workspace(nmf_plan* p) {
     return main + nmf_align_up(nmf_aux_workspace(p), 256);
 }
 
+// every call must run with the plan's device current (launches, function attributes and copies use the current device)
+int check_device(const nmf_plan* p) {
+    int d = -1;
+    if (cudaGetDevice(&d) != cudaSuccess) return NMF_ERR_CUDA;
+    return d == p->device ? NMF_OK : NMF_ERR_INVALID_ARG;
+}
+
 int check_ws(const nmf_plan* p) {
+    int rc = check_device(p);
+    if (rc) return rc;
     if (!p->ws || p->ws_bytes < p->ws_needed) return NMF_ERR_WORKSPACE;
     return NMF_OK;
 }
@@ -85,8 +94,13 @@ int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int ma
     cudaDeviceProp prop;
     if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return NMF_ERR_CUDA;
     if (prop.major != 10) return NMF_ERR_ARCH;
+    if (dev < 0 || dev >= NMF_MAX_DEVICES) return NMF_ERR_UNSUPPORTED;
     nmf_plan* p = new (std::nothrow) nmf_plan();
     if (!p) return NMF_ERR_INVALID_ARG;
+    if (cudaMallocHost(reinterpret_cast<void**>(&p->host_scratch), 8 * sizeof(double)) != cudaSuccess) {
+        delete p;
+        return NMF_ERR_CUDA;
+    }
     p->N = N; p->P = P; p->K = K; p->batch = batch; p->max_targets = max_targets;
     p->device = dev; p->num_sms = prop.multiProcessorCount;
     nmf_generic_configure(p);
@@ -129,6 +143,7 @@ int nmf_plan_destroy(nmf_plan* p) {
     if (!p) return NMF_ERR_INVALID_ARG;
     if (p->stage) cudaFree(p->stage);
     if (p->own_ws) cudaFree(p->own_ws);
+    if (p->host_scratch) cudaFreeHost(p->host_scratch);
     delete p;
     return NMF_OK;
 }
@@ -164,6 +179,8 @@ int nmf_subtract(nmf_plan* p, const float* H, const float* T, const float* C, co
     if (out == T || out == H) return NMF_ERR_INVALID_ARG;
     if (misaligned(H) || misaligned(T) || misaligned(C) || misaligned(out) || (om && misaligned(om)))
         return NMF_ERR_ALIGNMENT;
+    int rc = check_device(p);
+    if (rc) return rc;
     return nmf_aux_subtract(p, H, T, C, om, factor, fill, out, M);
 }
 
@@ -178,10 +195,34 @@ int nmf_objective(nmf_plan* p, const float* X, const float* Om, const float* W, 
     return nmf_aux_objective(p, X, Om, W, H, out_host);
 }
 
+int nmf_fit_tol(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int max_iters, int check_every,
+                double tol, int* iters_done, double* f_last) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!X || !Om || !W || !H || !iters_done || max_iters < 0 || check_every < 1 || !(tol >= 0.0)) return NMF_ERR_INVALID_ARG;
+    if (misaligned(X) || misaligned(Om) || misaligned(W) || misaligned(H)) return NMF_ERR_ALIGNMENT;
+    int rc = check_ws(p);
+    if (rc) return rc;
+    return nmf_aux_fit_tol(p, nmf_fit, X, Om, W, H, max_iters, check_every, tol, iters_done, f_last);
+}
+
+int nmf_derotate_stack(nmf_plan* p, const float* resid, const float* om, const float* angle_deg, int ny, int nx,
+                       float fill, float* out, int* count, int M) {
+    if (!p) return NMF_ERR_INVALID_ARG;
+    if (p->sticky) return p->sticky;
+    if (!resid || !angle_deg || !out || M < 1 || ny < 1 || nx < 1 || (long long)ny * nx != p->P) return NMF_ERR_INVALID_ARG;
+    if (out == resid) return NMF_ERR_INVALID_ARG;
+    if (misaligned(resid) || misaligned(out) || (om && misaligned(om))) return NMF_ERR_ALIGNMENT;
+    int rc = check_device(p);
+    if (rc) return rc;
+    return nmf_aux_derotate_stack(p, resid, om, angle_deg, ny, nx, fill, out, count, M);
+}
+
 int nmf_fit_host(nmf_plan* p, const float* Xh, const float* Oh, float* Wh, float* Hh, int iters) {
     if (!p) return NMF_ERR_INVALID_ARG;
     if (p->sticky) return p->sticky;
     if (!Xh || !Oh || !Wh || !Hh || iters < 0) return NMF_ERR_INVALID_ARG;
+    if (int rcd = check_device(p)) return rcd;
     const size_t np = nmf_align_up(sizeof(float) * (size_t)p->N * p->P, 256);
     const size_t nk = nmf_align_up(sizeof(float) * (size_t)p->N * p->K, 256);
     const size_t kp = nmf_align_up(sizeof(float) * (size_t)p->K * p->P, 256);
@@ -211,6 +252,7 @@ int nmf_project_subtract_host(nmf_plan* p, const float* H, const float* Th, cons
     if (!p) return NMF_ERR_INVALID_ARG;
     if (p->sticky) return p->sticky;
     if (!H || !Th || !Ch || !outh || M < 1 || M > p->max_targets || iters < 0) return NMF_ERR_INVALID_ARG;
+    if (int rcd = check_device(p)) return rcd;
     const size_t mp = nmf_align_up(sizeof(float) * (size_t)M * p->P, 256);
     const size_t mk = nmf_align_up(sizeof(float) * (size_t)M * p->K, 256);
     int rc = ensure_stage(p, 3 * mp + mk);
@@ -251,6 +293,8 @@ int nmf_ref_select(nmf_plan* p, const float* dist, int M, int n_sel, int* idx) {
     if (!p) return NMF_ERR_INVALID_ARG;
     if (p->sticky) return p->sticky;
     if (!dist || !idx || M < 1 || n_sel < 1 || n_sel > p->N) return NMF_ERR_INVALID_ARG;
+    int rc = check_device(p);
+    if (rc) return rc;
     return nmf_select_topn(p, dist, M, n_sel, idx);
 }
 

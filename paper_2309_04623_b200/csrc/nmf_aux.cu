@@ -1,5 +1,6 @@
-// nmf_aux.cu -- PSF subtraction and the diagnostic
-// objective of Eq. 2.
+// nmf_aux.cu -- PSF subtraction, the objective of Eq. 2 reduced on the device
+// in fp64 in a fixed order, the tolerance test of the stopping rule (8(f) NEXT-3) and
+// derotation + stacking of the residual frames (8(f) NEXT-4).
 #include "nmf_common.cuh"
 
 namespace {
@@ -114,10 +115,104 @@ k_objective(const float* __restrict__ X, const float* __restrict__ Om, const flo
     }
 }
 
+// fixed-order sum of the per-block partials: thread i adds partials i, i + 256, ... in order, thread 0 then adds the
+// 256 thread sums in order (bitwise reproducible); one block
+constexpr int RED_THREADS = 256;
+__global__ void __launch_bounds__(RED_THREADS)
+k_objective_reduce(const double* __restrict__ partial, int n, double* __restrict__ f_out) {
+    __shared__ double sh[RED_THREADS];
+    double a = 0.0;
+    for (int i = threadIdx.x; i < n; i += RED_THREADS) a += partial[i];
+    sh[threadIdx.x] = a;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double t = 0.0;
+        for (int i = 0; i < RED_THREADS; ++i) t += sh[i];
+        *f_out = t;
+    }
+}
+
+// stopping test of reading G21: stop = |f_prev - f_cur| < tol * f_prev; then f_prev <- f_cur.
+// res[0] = f_prev (in/out), res[1] = f_cur (in), res[2] = stop flag as a double (out)
+__global__ void k_tol_check(double* res, double tol) {
+    const double fp = res[0], fc = res[1];
+    res[2] = (fabs(fp - fc) < tol * fp) ? 1.0 : 0.0;
+    res[0] = fc;
+}
+
+// sine / cosine of an angle in degrees, exact at multiples of 90 degrees (reading G22): fold to the nearest multiple
+// of 90, evaluate the remainder |r| <= 45 degrees in fp64, rotate by the quadrant
+__device__ __forceinline__ void sincos_deg(double deg, double* s, double* c) {
+    double a = fmod(deg, 360.0);
+    if (a < 0.0) a += 360.0;
+    const int k = (int)floor(a / 90.0 + 0.5);
+    const double r = (a - 90.0 * k) * (3.14159265358979323846 / 180.0);
+    double sr, cr;
+    sincos(r, &sr, &cr);
+    switch (k & 3) {
+        case 0: *s = sr;  *c = cr;  break;
+        case 1: *s = cr;  *c = -sr; break;
+        case 2: *s = -sr; *c = -cr; break;
+        default: *s = -cr; *c = sr; break;
+    }
+}
+
+// derotate + stack (readings G22-G24): one output pixel per thread, 32 x 8 pixel tile per CTA; frame m rotated by
+// angle[m] about the pixel (ny / 2, nx / 2), bilinear over the neighbours with weight > 1e-6, a sample counts only if
+// all of those are inside the image and have omega > 0; out = mean over the frames with a sample, else `fill`.
+// Source coordinates and weights in fp64 (they decide which pixels are read), the weighted sum in fp32.
+constexpr int ROT_TX = 32, ROT_TY = 8, ROT_MC = 128;
+__global__ void __launch_bounds__(ROT_TX * ROT_TY)
+k_derotate_stack(const float* __restrict__ R, const float* __restrict__ om, const float* __restrict__ angle,
+                 int M, int ny, int nx, float fill, float* __restrict__ out, int* __restrict__ count) {
+    __shared__ double sn[ROT_MC], cs[ROT_MC];
+    const int tid = threadIdx.y * ROT_TX + threadIdx.x;
+    const int x = blockIdx.x * ROT_TX + threadIdx.x, y = blockIdx.y * ROT_TY + threadIdx.y;
+    const bool in = x < nx && y < ny;
+    const size_t P = (size_t)ny * nx;
+    const int cy = ny / 2, cx = nx / 2;
+    const double dx = x - cx, dy = y - cy;
+    float sum = 0.f;
+    int cnt = 0;
+    for (int m0 = 0; m0 < M; m0 += ROT_MC) {
+        const int mc = min(ROT_MC, M - m0);
+        __syncthreads();
+        if (tid < mc) sincos_deg((double)angle[m0 + tid], &sn[tid], &cs[tid]);
+        __syncthreads();
+        if (!in) continue;
+        for (int m = 0; m < mc; ++m) {
+            const double xs = cx + cs[m] * dx + sn[m] * dy;
+            const double ys = cy - sn[m] * dx + cs[m] * dy;
+            const double x0 = floor(xs), y0 = floor(ys);
+            const double fx = xs - x0, fy = ys - y0;
+            const double w[4] = {(1.0 - fx) * (1.0 - fy), fx * (1.0 - fy), (1.0 - fx) * fy, fx * fy};
+            const float* Rm = R + (size_t)(m0 + m) * P;
+            const float* om_m = om ? om + (size_t)(m0 + m) * P : nullptr;
+            bool valid = true;
+            float v = 0.f;
+#pragma unroll
+            for (int i = 0; i < 4; ++i) {
+                if (!(w[i] > 1e-6)) continue;
+                const double xi = x0 + (i & 1), yi = y0 + (i >> 1);
+                if (xi < 0 || xi >= nx || yi < 0 || yi >= ny) { valid = false; continue; }
+                const size_t j = (size_t)yi * nx + (size_t)xi;
+                if (om_m && !(__ldg(om_m + j) > 0.f)) { valid = false; continue; }
+                if (valid) v = fmaf((float)w[i], __ldg(Rm + j), v);     // (a masked pixel's value is never read)
+            }
+            if (valid) { sum += v; ++cnt; }
+        }
+    }
+    if (in) {
+        out[(size_t)y * nx + x] = cnt ? sum / (float)cnt : fill;
+        if (count) count[(size_t)y * nx + x] = cnt;
+    }
+}
+
 }  // namespace
 
 size_t nmf_aux_workspace(const nmf_plan* p) {
-    return sizeof(double) * (size_t)((p->P + OBJ_THREADS - 1) / OBJ_THREADS);
+    // objective partials (one double per block) + 4 doubles: f_prev, f_cur, stop flag, spare
+    return sizeof(double) * ((size_t)((p->P + OBJ_THREADS - 1) / OBJ_THREADS) + 4);
 }
 
 int nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C, const float* om,
@@ -133,28 +228,77 @@ int nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C
     return NMF_OK;
 }
 
-int nmf_aux_objective(nmf_plan* p, const float* X, const float* Om, const float* W, const float* H,
-                      double* out_host) {
+// scratch doubles at the very end of the workspace: [0] f_prev, [1] f_cur, [2] stop flag
+static double* aux_scratch(nmf_plan* p) {
+    return reinterpret_cast<double*>(static_cast<char*>(p->ws) + p->ws_needed) - 4;
+}
+
+// the cost of Eq. 2 at (W, H) into device memory `f_dev` (fp64, fixed-order: bitwise reproducible); asynchronous
+int nmf_aux_objective_dev(nmf_plan* p, const float* X, const float* Om, const float* W, const float* H, double* f_dev) {
     const unsigned grid = (unsigned)((p->P + OBJ_THREADS - 1) / OBJ_THREADS);
     const size_t smem = sizeof(float) * ((size_t)p->N * p->K + (size_t)p->K * OBJ_THREADS);
-    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
-    if (!attr_done) {
+    static bool attr_done[NMF_MAX_DEVICES] = {};   // function attributes are per device
+    if (!attr_done[p->device]) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_objective, cudaFuncAttributeMaxDynamicSharedMemorySize, 200 * 1024));
-        attr_done = true;
+        attr_done[p->device] = true;
     }
     // objective partials live at the tail of the workspace
     double* partial = reinterpret_cast<double*>(static_cast<char*>(p->ws) + (p->ws_needed - nmf_aux_workspace(p)));
     k_objective<<<grid, OBJ_THREADS, smem, p->stream>>>(X, Om, W, H, partial, p->N, p->P, p->K);
+    k_objective_reduce<<<1, RED_THREADS, 0, p->stream>>>(partial, (int)grid, f_dev);
+    p->launches += 2;
+    NMF_CUDA_TRY(p, cudaGetLastError());
+    return NMF_OK;
+}
+
+int nmf_aux_objective(nmf_plan* p, const float* X, const float* Om, const float* W, const float* H,
+                      double* out_host) {
+    double* sc = aux_scratch(p);
+    int rc = nmf_aux_objective_dev(p, X, Om, W, H, sc + 1);
+    if (rc) return rc;
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(p->host_scratch, sc + 1, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    NMF_CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    *out_host = p->host_scratch[0];
+    return NMF_OK;
+}
+
+// fit with the tolerance stop of reading G21: blocks of `check_every` iterations, each followed by the device-side
+// cost + stopping test; the host reads the 3-double result once per block (not per iteration)
+int nmf_aux_fit_tol(nmf_plan* p, int (*fit)(nmf_plan*, const float*, const float*, float*, float*, int),
+                    const float* X, const float* Om, float* W, float* H, int max_iters, int check_every, double tol,
+                    int* iters_done, double* f_last) {
+    double* sc = aux_scratch(p);
+    int rc = nmf_aux_objective_dev(p, X, Om, W, H, sc);            // f_prev = f_0
+    if (rc) return rc;
+    NMF_CUDA_TRY(p, cudaMemcpyAsync(p->host_scratch, sc, sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+    int it = 0;
+    bool checked = false;
+    while (it < max_iters) {
+        const int n = (max_iters - it < check_every) ? max_iters - it : check_every;
+        rc = fit(p, X, Om, W, H, n);
+        if (rc) return rc;
+        it += n;
+        if (n < check_every) break;                                // max_iters reached between two checks
+        rc = nmf_aux_objective_dev(p, X, Om, W, H, sc + 1);
+        if (rc) return rc;
+        k_tol_check<<<1, 1, 0, p->stream>>>(sc, tol);
+        p->launches++;
+        NMF_CUDA_TRY(p, cudaMemcpyAsync(p->host_scratch, sc, 3 * sizeof(double), cudaMemcpyDeviceToHost, p->stream));
+        NMF_CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+        checked = true;
+        if (p->host_scratch[2] != 0.0) break;
+    }
+    if (!checked) NMF_CUDA_TRY(p, cudaStreamSynchronize(p->stream));
+    *iters_done = it;
+    if (f_last) *f_last = p->host_scratch[0];
+    return NMF_OK;
+}
+
+int nmf_aux_derotate_stack(nmf_plan* p, const float* R, const float* om, const float* angle, int ny, int nx, float fill,
+                           float* out, int* count, int M) {
+    dim3 grid((nx + ROT_TX - 1) / ROT_TX, (ny + ROT_TY - 1) / ROT_TY), block(ROT_TX, ROT_TY);
+    k_derotate_stack<<<grid, block, 0, p->stream>>>(R, om, angle, M, ny, nx, fill, out, count);
     p->launches++;
     NMF_CUDA_TRY(p, cudaGetLastError());
-    double* host = nullptr;
-    NMF_CUDA_TRY(p, cudaMallocHost(&host, sizeof(double) * grid));
-    cudaError_t e = cudaMemcpyAsync(host, partial, sizeof(double) * grid, cudaMemcpyDeviceToHost, p->stream);
-    if (e == cudaSuccess) e = cudaStreamSynchronize(p->stream);
-    if (e != cudaSuccess) { cudaFreeHost(host); return nmf_cuda_fail(p, e); }
-    double f = 0.0;
-    for (unsigned i = 0; i < grid; ++i) f += host[i];   // fixed order
-    cudaFreeHost(host);
-    *out_host = f;
     return NMF_OK;
 }

@@ -44,6 +44,7 @@ struct nmf_plan {
     void* stage = nullptr;
     size_t stage_bytes = 0;
     void* own_ws = nullptr;       // workspace allocated by a *_host call when none was set
+    double* host_scratch = nullptr;   // 8 pinned doubles: results read back by nmf_objective / nmf_fit_tol
 };
 
 static inline int nmf_cuda_fail(nmf_plan* p, cudaError_t e) {
@@ -102,3 +103,10 @@ int    nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float
                         const float* om, const float* factor, float fill, float* out, int M);
 int    nmf_aux_objective(nmf_plan* p, const float* X, const float* Om, const float* W,
                          const float* H, double* out_host);
+int    nmf_aux_objective_dev(nmf_plan* p, const float* X, const float* Om, const float* W,
+                             const float* H, double* f_dev);
+int    nmf_aux_fit_tol(nmf_plan* p, int (*fit)(nmf_plan*, const float*, const float*, float*, float*, int),
+                       const float* X, const float* Om, float* W, float* H, int max_iters, int check_every,
+                       double tol, int* iters_done, double* f_last);
+int    nmf_aux_derotate_stack(nmf_plan* p, const float* R, const float* om, const float* angle, int ny, int nx,
+                              float fill, float* out, int* count, int M);

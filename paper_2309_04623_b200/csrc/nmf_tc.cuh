@@ -46,12 +46,14 @@ __device__ __forceinline__ bool mbar_try_wait_hint(uint64_t* bar, uint32_t parit
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity), "r"(ns) : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (launch error surfaced by the C-ABI) instead of hanging the GPU.
+// Bounded wait: a protocol bug traps (launch error surfaced by the C-ABI) instead of hanging the GPU.  The bound is
+// ~20 s of SM clock: far beyond any legitimate wait (a whole launch takes milliseconds) even when the context is
+// time-sliced or stopped in a debugger for a while.
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     if (mbar_try_wait(bar, parity)) return;
     const long long t0 = clock64();
     while (!mbar_try_wait_hint(bar, parity, 20000u)) {
-        if (clock64() - t0 > 4000000000LL) __trap();
+        if (clock64() - t0 > 40000000000LL) __trap();
     }
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
@@ -219,8 +221,8 @@ inline encode_fn_t encode_fn() {
     return fn;
 }
 
-// 2-D fp32 map over a row-major [rows, P] array, box [box_rows][box_px]
-inline bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, int box_rows, int box_px, bool swizzle64) {
+// 2-D fp32 map over a row-major [rows, P] array, box [box_rows][box_px], shared-memory swizzle 0 / 64 / 128 bytes
+inline bool make_map(CUtensorMap* m, const float* base, long long rows, long long P, int box_rows, int box_px, int swizzle_bytes) {
     encode_fn_t fn = encode_fn();
     if (!fn) return false;
     const cuuint64_t dims[2] = {(cuuint64_t)P, (cuuint64_t)rows};
@@ -228,7 +230,8 @@ inline bool make_map(CUtensorMap* m, const float* base, long long rows, long lon
     const cuuint32_t box[2] = {(cuuint32_t)box_px, (cuuint32_t)box_rows};
     const cuuint32_t estr[2] = {1, 1};
     return fn(m, CU_TENSOR_MAP_DATA_TYPE_FLOAT32, 2, const_cast<float*>(base), dims, strides, box, estr,
-              CU_TENSOR_MAP_INTERLEAVE_NONE, swizzle64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
+              CU_TENSOR_MAP_INTERLEAVE_NONE,
+              swizzle_bytes == 128 ? CU_TENSOR_MAP_SWIZZLE_128B : swizzle_bytes == 64 ? CU_TENSOR_MAP_SWIZZLE_64B : CU_TENSOR_MAP_SWIZZLE_NONE,
               CU_TENSOR_MAP_L2_PROMOTION_L2_128B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE) == CUDA_SUCCESS;
 }
 

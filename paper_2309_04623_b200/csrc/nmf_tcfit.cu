@@ -586,9 +586,9 @@ namespace {
 int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* H, int rows, int iters, int batch, bool proj) {
     TcArgs a;
     const long long trows = (long long)batch * rows;
-    if (!make_map(&a.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) ||
-        !make_map(&a.mXh, X, trows, p->P, FCH, TILE, false) || !make_map(&a.mOh, Om, trows, p->P, FCH, TILE, false) ||
-        !make_map(&a.mXw, X, trows, p->P, 128, PCH, true) || !make_map(&a.mOw, Om, trows, p->P, 128, PCH, true)) {
+    if (!make_map(&a.mH, H, (long long)batch * p->K, p->P, 32, TILE, 0) ||
+        !make_map(&a.mXh, X, trows, p->P, FCH, TILE, 0) || !make_map(&a.mOh, Om, trows, p->P, FCH, TILE, 0) ||
+        !make_map(&a.mXw, X, trows, p->P, 128, PCH, 64) || !make_map(&a.mOw, Om, trows, p->P, 128, PCH, 64)) {
         if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
         return NMF_ERR_CUDA;
     }

@@ -36,18 +36,22 @@ constexpr int FCH = 16;                   // frames per H-step chunk (one UMMA K
 constexpr int PCH = 16;                   // pixels per W-step chunk
 constexpr int NCH2 = TILE / PCH;
 constexpr int HS_SB = 16 * 128;           // [128 rows][comps] piece buffers: bytes between 8-component groups
-constexpr int SLOT = 16384;               // ring slot bytes
+constexpr int SLOT = 16384;               // ring slot bytes (k_tc_h)
+constexpr int PSW = 32;                   // k_tc_w: pixels per ring slot = one super-chunk (two W-step chunks)
+constexpr int NSW = TILE / PSW;           // k_tc_w: X / Omega slots per tile
+constexpr int SLOTW = 32768;              // k_tc_w ring slot bytes: [64 comps][128 px] of H, or [128 frames][32 px] of X and of Omega
 constexpr int MAX_SLOTS = 8;
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 struct SplitArgs {
-    CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px]
-    CUtensorMap mX, mO;        // X, Om [B*rows, P]: box [16 frames][128 px] (k_tc_h) or [128 frames][16 px], 64-byte swizzle (k_tc_w)
+    CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px] (k_tc_h) or [64 comps][128 px] (k_tc_w)
+    CUtensorMap mX, mO;        // X, Om [B*rows, P]: box [16 frames][128 px] (k_tc_h) or [128 frames][32 px], 128-byte swizzle
+                               // (k_tc_w: full 128-byte lines from HBM; 64-byte rows ran the kernel at a quarter of the HBM rate)
     const float* W; float* H; float* slab;
     int N, K; long long P; long long n_tiles;
     int NF;                    // frames padded to a multiple of 16
     int NC;                    // H-step chunks = NF / 16
-    int KH;                    // 32-component TMA slots of the H tile
+    int KH;                    // TMA slots of the H tile (32 components each in k_tc_h, 64 in k_tc_w)
     int NS;                    // ring slots
 };
 
@@ -365,7 +369,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     const long long P = g.P;
     constexpr int HS_BYTES = (KP / 8) * HS_SB;          // one BF16 piece of the H tile / of the M tile's W rows
     unsigned char* ring = smem;
-    unsigned char* hs_p = ring + (size_t)g.NS * SLOT;   // 3 pieces of the H tile, [pixel][comp]
+    unsigned char* hs_p = ring + (size_t)g.NS * SLOTW;  // 3 pieces of the H tile, [pixel][comp]
     unsigned char* ws3_p = hs_p + 3 * HS_BYTES;         // piece 3 of this M tile's rows of W (NPT == 2 only)
     uint64_t* bars = reinterpret_cast<uint64_t*>(ws3_p + (NPT == 2 ? HS_BYTES : 0));
     uint32_t* tptr = reinterpret_cast<uint32_t*>(bars + B_COUNT);
@@ -382,7 +386,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
         mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1);
         mbar_init(&bars[B_P0], 4); mbar_init(&bars[B_P1], 4); mbar_init(&bars[B_G0], 1); mbar_init(&bars[B_G1], 1);
         mbar_init(&bars[B_DONE], 1);
-        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 4); }
+        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], EW_WARPS); }
         mbar_fence_init();
     }
     if (warp == W_MMA) tmem_alloc(tptr, 512);
@@ -392,7 +396,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     tc_fence_after();
     const uint32_t tmem = *tptr;
     const uint32_t hs_s = smem_u32(hs_p), ws3_s = smem_u32(ws3_p), ring_s = smem_u32(ring);
-    const uint32_t slots_per_tile = (uint32_t)(KH + NCH2);
+    const uint32_t slots_per_tile = (uint32_t)(KH + NSW);
     constexpr int NSC2 = NCH2 / 2;
 
     if (warp < EW_WARPS) {
@@ -434,7 +438,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                 uint32_t par;
                 const uint32_t s = rc.slot(seq, par);
                 mbar_wait(&bars[B_EMPTY + s], par ^ 1u);
-                mbar_expect_tx(&bars[B_FULL + s], SLOT);
+                mbar_expect_tx(&bars[B_FULL + s], SLOTW);
                 ++seq;
                 return s;
             };
@@ -442,12 +446,12 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                 const int p0 = (int)(tile * TILE);
                 for (int h = 0; h < KH; ++h) {
                     const uint32_t s = acquire();
-                    tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
+                    tma_load_2d(ring_s + s * SLOTW, &g.mH, p0, b * K + 64 * h, &bars[B_FULL + s]);
                 }
-                for (int c = 0; c < NCH2; ++c) {         // the M tile's 128 rows of X and Omega, 16 px at a time
+                for (int c = 0; c < NSW; ++c) {          // the M tile's 128 rows of X and Omega, 32 px (one super-chunk) at a time
                     const uint32_t s = acquire();
-                    tma_load_2d(ring_s + s * SLOT, &g.mX, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
-                    tma_load_2d(ring_s + s * SLOT + 128 * PCH * 4, &g.mO, p0 + PCH * c, b * N + 128 * m, &bars[B_FULL + s]);
+                    tma_load_2d(ring_s + s * SLOTW, &g.mX, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
+                    tma_load_2d(ring_s + s * SLOTW + 128 * PSW * 4, &g.mO, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
                 }
             }
         }
@@ -523,7 +527,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             uint32_t par;
             const uint32_t s = rc.slot(seq, par);
             mbar_wait(&bars[B_FULL + s], par);
-            return ring + (size_t)s * SLOT;
+            return ring + (size_t)s * SLOTW;
         };
         auto release = [&](uint32_t seq) {
             __syncwarp();
@@ -537,21 +541,25 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
         uint32_t sq = 0;
         bool first = true;
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
-            // ---- H0: the (new) H tile is split into Hs[pixel][comp]; thread = pixel t; group g takes slots g, g + 2, ...
+            // ---- H0: the (new) H tile is split into Hs[pixel][comp]; thread = pixel t; a slot holds 64 components,
+            // group g takes components 64 h + 32 g .. + 31 of slot h
             if (!first) wait(B_DONE);                    // every MMA of the previous tile is complete: Hs is free
             first = false;
-            for (int h = grp; h < KH; h += 2) {
-                const float* hsl = reinterpret_cast<const float*>(wait_full(sq + h));
-                uint32_t p1[16], p2[16], p3[16];
-                split_slot32(hsl, t, 32 * h, K, p1, p2, p3);
-                release(sq + h);
+            for (int h = 0; h < KH; ++h) {
+                const float* hsl = reinterpret_cast<const float*>(wait_full(sq + h)) + (32 * grp) * TILE;
+                const int hh = 2 * h + grp;              // 32-component block
+                if (32 * hh < KP) {
+                    uint32_t p1[16], p2[16], p3[16];
+                    split_slot32(hsl, t, 32 * hh, K, p1, p2, p3);
 #pragma unroll
-                for (int gq = 0; gq < 4; ++gq)
-                    if (4 * h + gq < KP / 8) {
-                        st_piece_smem(hs_p, t, 4 * h + gq, &p1[4 * gq]);
-                        st_piece_smem(hs_p + HS_BYTES, t, 4 * h + gq, &p2[4 * gq]);
-                        st_piece_smem(hs_p + 2 * HS_BYTES, t, 4 * h + gq, &p3[4 * gq]);
-                    }
+                    for (int gq = 0; gq < 4; ++gq)
+                        if (4 * hh + gq < KP / 8) {
+                            st_piece_smem(hs_p, t, 4 * hh + gq, &p1[4 * gq]);
+                            st_piece_smem(hs_p + HS_BYTES, t, 4 * hh + gq, &p2[4 * gq]);
+                            st_piece_smem(hs_p + 2 * HS_BYTES, t, 4 * hh + gq, &p3[4 * gq]);
+                        }
+                }
+                release(sq + h);
             }
             fence_proxy_async();
             warp_arrive(B_HS);
@@ -559,17 +567,17 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             // ---- steps: super-chunk j = chunks 2j + grp; thread = (frame 128 m + t, 16 pixels) ----
             bool pending = false;
             for (int j = 0; j < NSC2; ++j) {
-                const int c = 2 * j + grp;
-                const uint32_t seq = sq + KH + c;
-                const unsigned char* xsl = wait_full(seq);           // X rows at +0, Omega rows at +8 KB
+                const uint32_t seq = sq + KH + j;        // both groups read the super-chunk's slot: group g its pixels 16 g .. 16 g + 15
+                const unsigned char* xsl = wait_full(seq);           // X rows (128 bytes each, 128-byte swizzle) at +0, Omega rows at +16 KB
                 float x[16], o[16];
                 if (active) {
                     if (fr < N) {
-                        const int sw = (t >> 1) & 3;
+                        const int sw = t & 7;
 #pragma unroll
                         for (int ch = 0; ch < 4; ++ch) {
-                            const float4 xv = *reinterpret_cast<const float4*>(xsl + t * 64 + ((ch ^ sw) << 4));
-                            const float4 ov = *reinterpret_cast<const float4*>(xsl + 128 * PCH * 4 + t * 64 + ((ch ^ sw) << 4));
+                            const int cs = ((4 * grp + ch) ^ sw) << 4;
+                            const float4 xv = *reinterpret_cast<const float4*>(xsl + t * 128 + cs);
+                            const float4 ov = *reinterpret_cast<const float4*>(xsl + 128 * PSW * 4 + t * 128 + cs);
                             x[4 * ch] = xv.x; x[4 * ch + 1] = xv.y; x[4 * ch + 2] = xv.z; x[4 * ch + 3] = xv.w;
                             o[4 * ch] = ov.x; o[4 * ch + 1] = ov.y; o[4 * ch + 2] = ov.z; o[4 * ch + 3] = ov.w;
                         }
@@ -666,8 +674,8 @@ inline size_t smem_fixed_h(int NF, int KP) {
 inline size_t smem_fixed_w(int KP) {
     return (size_t)(3 + (npt_w(KP) == 2 ? 1 : 0)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
 }
-inline int slots_for(size_t fixed) {
-    long long ns = ((long long)SMEM_MAX - (long long)fixed) / SLOT;
+inline int slots_for(size_t fixed, int slot_bytes) {
+    long long ns = ((long long)SMEM_MAX - (long long)fixed) / slot_bytes;
     return (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
 }
 
@@ -707,19 +715,19 @@ int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, 
     SplitArgs h{}, w{};
     h.W = w.W = W; h.H = w.H = H; w.slab = h.slab = reinterpret_cast<float*>(p->ws);
     h.N = w.N = rows; h.K = w.K = p->K; h.P = w.P = p->P; h.n_tiles = w.n_tiles = n_tiles;
-    h.NF = w.NF = (rows + FCH - 1) / FCH * FCH; h.NC = w.NC = h.NF / FCH; h.KH = w.KH = (p->K + 31) / 32;
-    h.NS = slots_for(smem_fixed_h(h.NF, KP)); w.NS = slots_for(smem_fixed_w(KP));
-    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) &&
-              make_map(&w.mX, X, trows, p->P, 128, PCH, true) && make_map(&w.mO, Om, trows, p->P, 128, PCH, true);
-    if (fit) ok = ok && make_map(&h.mH, H, (long long)batch * p->K, p->P, 32, TILE, false) &&
-                  make_map(&h.mX, X, trows, p->P, FCH, TILE, false) && make_map(&h.mO, Om, trows, p->P, FCH, TILE, false);
+    h.NF = w.NF = (rows + FCH - 1) / FCH * FCH; h.NC = w.NC = h.NF / FCH; h.KH = (p->K + 31) / 32; w.KH = (p->K + 63) / 64;
+    h.NS = slots_for(smem_fixed_h(h.NF, KP), SLOT); w.NS = slots_for(smem_fixed_w(KP), SLOTW);
+    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 64, TILE, 0) &&
+              make_map(&w.mX, X, trows, p->P, 128, PSW, 128) && make_map(&w.mO, Om, trows, p->P, 128, PSW, 128);
+    if (fit) ok = ok && make_map(&h.mH, H, (long long)batch * p->K, p->P, 32, TILE, 0) &&
+                  make_map(&h.mX, X, trows, p->P, FCH, TILE, 0) && make_map(&h.mO, Om, trows, p->P, FCH, TILE, 0);
     if (!ok) {
         if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
         return NMF_ERR_CUDA;
     }
     const int ctas_h = even_ctas(n_tiles, p->num_sms / batch);
     const int ctas_w = even_ctas(n_tiles, p->num_sms / (batch * MT));
-    const size_t smem_h = smem_fixed_h(h.NF, KP) + (size_t)h.NS * SLOT, smem_w = smem_fixed_w(KP) + (size_t)w.NS * SLOT;
+    const size_t smem_h = smem_fixed_h(h.NF, KP) + (size_t)h.NS * SLOT, smem_w = smem_fixed_w(KP) + (size_t)w.NS * SLOTW;
     const int nk = rows * p->K;
     for (int it = 0; it < iters; ++it) {
         if (fit) {
@@ -741,7 +749,7 @@ void nmf_tcsplit_configure(nmf_plan* p) {
     if (p->K > 128 || p->N > 256) return;
     if (p->P + TILE >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
     const int KP = kp_of(p->K), NF = (p->N + FCH - 1) / FCH * FCH;
-    if (slots_for(smem_fixed_h(NF, KP)) < 2 || slots_for(smem_fixed_w(KP)) < 3) return;
+    if (slots_for(smem_fixed_h(NF, KP), SLOT) < 2 || slots_for(smem_fixed_w(KP), SLOTW) < 2) return;
     p->s_ok = true;
 }
 

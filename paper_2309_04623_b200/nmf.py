@@ -24,7 +24,7 @@ SYMBOLS = (
     "nmf_plan_create", "nmf_plan_workspace_bytes", "nmf_plan_set_workspace", "nmf_plan_set_stream",
     "nmf_plan_set_variant", "nmf_plan_get_variant", "nmf_plan_destroy", "nmf_fit", "nmf_fit_batched",
     "nmf_project", "nmf_subtract", "nmf_objective", "nmf_fit_host", "nmf_project_subtract_host",
-    "nmf_ref_distance", "nmf_ref_select",
+    "nmf_ref_distance", "nmf_ref_select", "nmf_fit_tol", "nmf_derotate_stack",
     "nmf_plan_launch_count", "nmf_status_string", "nmf_plan_last_cuda_error",
 )
 
@@ -61,6 +61,9 @@ def lib():
         L.nmf_objective.argtypes = [_vp, _vp, _vp, _vp, _vp, ctypes.POINTER(ctypes.c_double)]
         L.nmf_ref_distance.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _vp]
         L.nmf_ref_select.argtypes = [_vp, _vp, _ci, _ci, _vp]
+        L.nmf_fit_tol.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci, _ci, ctypes.c_double, ctypes.POINTER(_ci),
+                                  ctypes.POINTER(ctypes.c_double)]
+        L.nmf_derotate_stack.argtypes = [_vp, _vp, _vp, _vp, _ci, _ci, _cf, _vp, _vp, _ci]
         L.nmf_fit_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _ci]
         L.nmf_project_subtract_host.argtypes = [_vp, _vp, _vp, _vp, _vp, _cf, _vp, _ci, _ci]
         L.nmf_plan_launch_count.argtypes = [_vp]; L.nmf_plan_launch_count.restype = _cll
@@ -111,6 +114,10 @@ class Plan:
             raise NMFError(rc, lib().nmf_plan_last_cuda_error(self._h).decode() if self._h else "")
 
     def _sync_stream(self):
+        """Hand torch's current stream of the plan's device to the plan and make that device current (the library
+        checks it: a plan only works with its own device current)."""
+        if torch.cuda.current_device() != self.device.index:
+            torch.cuda.set_device(self.device)
         self._check(lib().nmf_plan_set_stream(self._h, torch.cuda.current_stream(self.device).cuda_stream))
 
     @property
@@ -137,6 +144,29 @@ class Plan:
         self._sync_stream()
         self._check(lib().nmf_fit(self._h, _dev(X, (self.N, self.P)), _dev(Omega, (self.N, self.P)),
                                   _dev(W, (self.N, self.K)), _dev(H, (self.K, self.P)), iters))
+
+    def fit_tol(self, X, Omega, W, H, max_iters: int, check_every: int, tol: float):
+        """nmf_fit_tol: fit with the tolerance stop.  Returns (iterations done, cost at the last check)."""
+        done, f = _ci(0), ctypes.c_double(0.0)
+        self._sync_stream()
+        with torch.cuda.device(self.device):
+            self._check(lib().nmf_fit_tol(self._h, _dev(X, (self.N, self.P)), _dev(Omega, (self.N, self.P)),
+                                          _dev(W, (self.N, self.K)), _dev(H, (self.K, self.P)), max_iters,
+                                          check_every, float(tol), ctypes.byref(done), ctypes.byref(f)))
+        return done.value, f.value
+
+    def derotate_stack(self, resid, omega, angle_deg, ny: int, nx: int, fill: float = 0.0, with_count: bool = False):
+        """nmf_derotate_stack: rotate the M residual frames by angle_deg [M] and average the valid samples."""
+        M = resid.shape[0]
+        out = torch.empty(self.P, dtype=torch.float32, device=self.device)
+        cnt = torch.empty(self.P, dtype=torch.int32, device=self.device) if with_count else None
+        self._sync_stream()
+        with torch.cuda.device(self.device):
+            self._check(lib().nmf_derotate_stack(self._h, _dev(resid, (M, self.P)),
+                                                 None if omega is None else _dev(omega, (M, self.P)),
+                                                 _dev(angle_deg, (M,)), ny, nx, float(fill), out.data_ptr(),
+                                                 None if cnt is None else cnt.data_ptr(), M))
+        return (out, cnt) if with_count else out
 
     def fit_batched(self, X, Omega, W, H, iters: int):
         B = self.batch
