@@ -144,6 +144,8 @@ int nmf_plan_destroy(nmf_plan* p) {
     if (p->stage) cudaFree(p->stage);
     if (p->own_ws) cudaFree(p->own_ws);
     if (p->host_scratch) cudaFreeHost(p->host_scratch);
+    if (p->g_exec) cudaGraphExecDestroy(p->g_exec);
+    if (p->cap_stream) cudaStreamDestroy(p->cap_stream);
     delete p;
     return NMF_OK;
 }

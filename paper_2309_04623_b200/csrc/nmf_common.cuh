@@ -45,6 +45,13 @@ struct nmf_plan {
     size_t stage_bytes = 0;
     void* own_ws = nullptr;       // workspace allocated by a *_host call when none was set
     double* host_scratch = nullptr;   // 8 pinned doubles: results read back by nmf_objective / nmf_fit_tol
+    // iteration loop as a CUDA graph (nmf_run_iterations): one instantiated graph of `g_unroll` iterations, kept
+    // while the same call (kernel family, buffers, shape) is repeated
+    cudaStream_t cap_stream = nullptr;    // plan-owned stream the graph is captured on (the legacy default stream cannot be)
+    cudaGraphExec_t g_exec = nullptr;
+    const void* g_key[6] = {nullptr, nullptr, nullptr, nullptr, nullptr, nullptr};
+    int g_rows = 0, g_batch = 0, g_unroll = 0, g_kind = 0;
+    long long g_launches = 0;             // kernel launches of one replay
 };
 
 static inline int nmf_cuda_fail(nmf_plan* p, cudaError_t e) {
@@ -56,6 +63,62 @@ static inline int nmf_cuda_fail(nmf_plan* p, cudaError_t e) {
          if (_e != cudaSuccess) return nmf_cuda_fail((plan), _e); } while (0)
 
 static inline size_t nmf_align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// ---------------------------------------------------------------------------
+// iteration loop without per-launch host work
+// ---------------------------------------------------------------------------
+// Runs `iters` repetitions of `one()` -- which enqueues ONE iteration's kernels on plan->stream and returns an NMF
+// status -- in stream order on plan->stream.  From NMF_GRAPH_MIN iterations up, min(iters, NMF_GRAPH_UNROLL)
+// repetitions are captured once into a CUDA graph (on a plan-owned capture stream), instantiated, and replayed
+// iters / unroll times; the remainder is enqueued directly.  The instantiated graph is kept in the plan and reused
+// while the same call (kind, buffers, rows, batch) comes again.  Inside someone else's capture the plain loop runs.
+#define NMF_GRAPH_MIN 8
+#define NMF_GRAPH_UNROLL 50
+template <class F>
+static inline int nmf_run_iterations(nmf_plan* p, int kind, const void* k0, const void* k1, const void* k2, const void* k3,
+                                     const void* k4, int rows, int batch, int iters, F one) {
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    const bool capturing = cudaStreamIsCapturing(p->stream, &cs) != cudaSuccess || cs != cudaStreamCaptureStatusNone;
+    if (capturing) (void)cudaGetLastError();
+    int done = 0;
+    if (!capturing && iters >= NMF_GRAPH_MIN) {
+        const int unroll = iters < NMF_GRAPH_UNROLL ? iters : NMF_GRAPH_UNROLL;
+        const void* key[6] = {k0, k1, k2, k3, k4, reinterpret_cast<const void*>(p->ws)};
+        bool hit = p->g_exec && p->g_kind == kind && p->g_rows == rows && p->g_batch == batch && p->g_unroll == unroll;
+        for (int i = 0; i < 6 && hit; ++i) hit = p->g_key[i] == key[i];
+        if (!hit) {
+            if (p->g_exec) { cudaGraphExecDestroy(p->g_exec); p->g_exec = nullptr; }
+            if (!p->cap_stream) NMF_CUDA_TRY(p, cudaStreamCreateWithFlags(&p->cap_stream, cudaStreamNonBlocking));
+            cudaStream_t user = p->stream;
+            const long long l0 = p->launches;
+            NMF_CUDA_TRY(p, cudaStreamBeginCapture(p->cap_stream, cudaStreamCaptureModeThreadLocal));
+            p->stream = p->cap_stream;
+            int rc = NMF_OK;
+            for (int u = 0; u < unroll && rc == NMF_OK; ++u) rc = one();
+            p->stream = user;
+            cudaGraph_t graph = nullptr;
+            cudaError_t e = cudaStreamEndCapture(p->cap_stream, &graph);
+            p->g_launches = p->launches - l0;
+            p->launches = l0;
+            if (rc != NMF_OK) { if (graph) cudaGraphDestroy(graph); return rc; }
+            NMF_CUDA_TRY(p, e);
+            e = cudaGraphInstantiate(&p->g_exec, graph, 0);
+            cudaGraphDestroy(graph);
+            if (e != cudaSuccess) { p->g_exec = nullptr; return nmf_cuda_fail(p, e); }
+            for (int i = 0; i < 6; ++i) p->g_key[i] = key[i];
+            p->g_kind = kind; p->g_rows = rows; p->g_batch = batch; p->g_unroll = unroll;
+        }
+        for (; done + p->g_unroll <= iters; done += p->g_unroll) {
+            NMF_CUDA_TRY(p, cudaGraphLaunch(p->g_exec, p->stream));
+            p->launches += p->g_launches;
+        }
+    }
+    for (; done < iters; ++done) {
+        int rc = one();
+        if (rc) return rc;
+    }
+    return NMF_OK;
+}
 
 // ---------------------------------------------------------------------------
 // launchers implemented in the .cu files (all enqueue on plan->stream)

@@ -322,12 +322,12 @@ bool nmf_fused_available(const nmf_plan* p) { return p->f_kp != 0; }
 int nmf_fused_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
     if (!p->f_kp) return NMF_ERR_UNSUPPORTED;
     const int kcp = round4(p->f_kp);
-    for (int it = 0; it < iters; ++it) {
+    int rcl = nmf_run_iterations(p, 20, X, Om, W, H, nullptr, p->N, batch, iters, [&]() -> int {
 #define CALL_F(KC) { int rc = launch<KC>(p, X, Om, W, H, batch); if (rc) return rc; }
         FUSED_DISPATCH(p->f_kp, CALL_F);
-        int rc = nmf_launch_w_update(p, reinterpret_cast<const float*>(p->ws), W, p->N, p->K, kcp, p->f_ctas, batch);
-        if (rc) return rc;
-    }
+        return nmf_launch_w_update(p, reinterpret_cast<const float*>(p->ws), W, p->N, p->K, kcp, p->f_ctas, batch);
+    });
+    if (rcl) return rcl;
     NMF_CUDA_TRY(p, cudaGetLastError());
     return NMF_OK;
 }

@@ -404,12 +404,14 @@ int nmf_launch_w_update(nmf_plan* p, const float* slab, float* W, int rows, int 
 int nmf_generic_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters,
                     int batch) {
     const int parts = batch == p->batch ? p->g_parts_fit : parts_for(p, p->N, batch);
-    for (int it = 0; it < iters; ++it) {
+    int rcl = nmf_run_iterations(p, 10, X, Om, W, H, nullptr, p->N, batch, iters, [&]() -> int {
 #define CALL_H(KC) { int rc = launch_h<KC>(p, X, Om, W, H, batch); if (rc) return rc; }
         DISPATCH_KC(p, CALL_H);
 #define CALL_W(KC) { int rc = launch_w<KC>(p, X, Om, W, H, p->N, parts, batch); if (rc) return rc; }
         DISPATCH_KC(p, CALL_W);
-    }
+        return NMF_OK;
+    });
+    if (rcl) return rcl;
     NMF_CUDA_TRY(p, cudaGetLastError());
     return NMF_OK;
 }
@@ -417,10 +419,12 @@ int nmf_generic_fit(nmf_plan* p, const float* X, const float* Om, float* W, floa
 int nmf_generic_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C,
                         int M, int iters) {
     const int parts = parts_for(p, M, 1);
-    for (int it = 0; it < iters; ++it) {
+    int rcl = nmf_run_iterations(p, 11, T, om, C, H, nullptr, M, 1, iters, [&]() -> int {
 #define CALL_P(KC) { int rc = launch_w<KC>(p, T, om, C, H, M, parts, 1); if (rc) return rc; }
         DISPATCH_KC(p, CALL_P);
-    }
+        return NMF_OK;
+    });
+    if (rcl) return rcl;
     NMF_CUDA_TRY(p, cudaGetLastError());
     return NMF_OK;
 }

@@ -46,14 +46,15 @@ __device__ __forceinline__ bool mbar_try_wait_hint(uint64_t* bar, uint32_t parit
         : "=r"(ok) : "r"(smem_u32(bar)), "r"(parity), "r"(ns) : "memory");
     return ok != 0;
 }
-// Bounded wait: a protocol bug traps (launch error surfaced by the C-ABI) instead of hanging the GPU.  The bound is
-// ~20 s of SM clock: far beyond any legitimate wait (a whole launch takes milliseconds) even when the context is
-// time-sliced or stopped in a debugger for a while.
+// Bounded wait: a protocol bug traps (launch error surfaced by the C-ABI) instead of hanging the GPU.  Each failed
+// probe has already slept in hardware for the try_wait time limit, so the loop is two instructions per wake-up (the
+// suspend-time-hint form compiles to TRYWAIT + NANOSLEEP.SYNCS + a second probe and woke about twenty times per
+// wait: a third of all instructions the element-wise warps issued); 2^26 failed probes are far beyond any legitimate
+// wait (a whole launch takes milliseconds).
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
-    if (mbar_try_wait(bar, parity)) return;
-    const long long t0 = clock64();
-    while (!mbar_try_wait_hint(bar, parity, 20000u)) {
-        if (clock64() - t0 > 40000000000LL) __trap();
+    uint32_t n = 0;
+    while (!mbar_try_wait(bar, parity)) {
+        if (++n > (1u << 26)) __trap();
     }
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
@@ -67,6 +68,12 @@ __device__ __forceinline__ void tma_load_2d(uint32_t smem_dst, const void* tmap,
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
+}
+// The same box is only brought into L2 (no shared-memory destination, no completion to wait for): issued a few tiles
+// ahead of the load, so that the bytes in flight from HBM wait in L2 and not in ring slots.
+__device__ __forceinline__ void tma_prefetch_l2_2d(const void* tmap, int x, int y) {
+    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];"
+                 ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(x), "r"(y) : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");
@@ -201,6 +208,29 @@ __device__ __forceinline__ void ew16(const float (&x)[16], const float (&o)[16],
         split3_pair(r0, r1, R1[i], R2[i], e[O_R3 + i]);
     }
     tmem_st8(zcol, R1); tmem_st8(zcol + 8, R2);
+}
+
+// The same stage for 8 consecutive elements (half a chunk), for the kernels that keep more chunks in flight with
+// fewer registers per thread: every piece comes back as 4 words (columns 4 h .. 4 h + 3 of its 8-column block for
+// half h).
+struct Ew8 { uint32_t r1[4], r2[4], r3[4], q1[4], q2[4], q3[4]; };
+__device__ __forceinline__ void ew8(const float (&x)[8], const float (&o)[8], const uint32_t* s, Ew8& w) {
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+        const float o0 = o[2 * i], o1 = o[2 * i + 1];
+        const float q0 = o0 > 0.f ? o0 * x[2 * i] : 0.f;
+        const float q1 = o1 > 0.f ? o1 * x[2 * i + 1] : 0.f;
+        const float r0 = o0 * __uint_as_float(s[2 * i]);          // S is finite: Omega == 0 gives exactly 0
+        const float r1 = o1 * __uint_as_float(s[2 * i + 1]);
+        split3_pair(q0, q1, w.q1[i], w.q2[i], w.q3[i]);
+        split3_pair(r0, r1, w.r1[i], w.r2[i], w.r3[i]);
+    }
+}
+// half h of a chunk's pieces -> TMEM: R1, R2 back over S in place (`zcol`), R3 and the Q pieces into the E block `ecol`
+__device__ __forceinline__ void ew8_store(uint32_t zcol, uint32_t ecol, int h, const Ew8& w) {
+    tmem_st4(zcol + 4 * h, w.r1); tmem_st4(zcol + 8 + 4 * h, w.r2);
+    tmem_st4(ecol + O_R3 + 4 * h, w.r3); tmem_st4(ecol + O_Q1 + 4 * h, w.q1);
+    tmem_st4(ecol + O_Q2 + 4 * h, w.q2); tmem_st4(ecol + O_Q3 + 4 * h, w.q3);
 }
 
 // ---------------------------------------------------------------- host: tensor maps

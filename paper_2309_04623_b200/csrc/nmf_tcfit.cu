@@ -538,11 +538,11 @@ size_t tc_smem_fixed(int NF) { return (size_t)3 * NF * 128 + 3 * HS_BYTES + B_CO
 
 template <int KS, int PLACE>
 cudaError_t launch_kp(const TcArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
-    static bool attr_done[64] = {};                      // function attributes are per device
-    if (device < 0 || device >= 64 || !attr_done[device]) {
+    static bool attr_done[NMF_MAX_DEVICES] = {};                      // function attributes are per device
+    if (device < 0 || device >= NMF_MAX_DEVICES || !attr_done[device]) {
         cudaError_t e = cudaFuncSetAttribute(k_tc_iter<KS, PLACE>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
         if (e != cudaSuccess) return e;
-        if (device >= 0 && device < 64) attr_done[device] = true;
+        if (device >= 0 && device < NMF_MAX_DEVICES) attr_done[device] = true;
     }
     k_tc_iter<KS, PLACE><<<grid, PLACE ? 384 : 320, smem, st>>>(a);
     return cudaSuccess;
@@ -606,7 +606,7 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
     const bool place = a.MT == 2 && rows <= 224 && KS == 4;
     const size_t smem = tc_smem_fixed(a.NF) + (size_t)a.NS * SLOT;
     const dim3 grid(p->t_ctas, batch);
-    for (int it = 0; it < iters; ++it) {
+    int rc = nmf_run_iterations(p, proj ? 31 : 30, X, Om, W, H, nullptr, rows, batch, iters, [&]() -> int {
         cudaError_t e;
         switch (KS) {
             case 1: e = launch_ks<1>(a, grid, smem, p->stream, place, p->device); break;
@@ -616,9 +616,9 @@ int tc_run(nmf_plan* p, const float* X, const float* Om, float* W, const float* 
         }
         NMF_CUDA_TRY(p, e);
         p->launches++;
-        int rc = nmf_launch_w_update(p, a.slab, W, rows, p->K, KP, p->t_ctas, batch);
-        if (rc) return rc;
-    }
+        return nmf_launch_w_update(p, a.slab, W, rows, p->K, KP, p->t_ctas, batch);
+    });
+    if (rc) return rc;
     NMF_CUDA_TRY(p, cudaGetLastError());
     return NMF_OK;
 }

@@ -1,26 +1,28 @@
 // nmf_tcsplit.cu -- the two half-steps of Eq. 3 as two persistent tcgen05 kernels, K <= 128.
 //
 // The fused kernel of nmf_tcfit.cu keeps Num/Den, S, the piece buffers AND the persistent W-phase accumulators
-// of two 128-frame M tiles in the 512 TMEM columns, and W and the H tile pieces in shared memory: that fills both
-// memories at K = 64 and leaves no column to feed the H-phase S stage from TMEM.  Here the iteration is split:
+// of two 128-frame M tiles in the 512 TMEM columns: that leaves no column to feed the H-phase S stage from TMEM and
+// room for only two chunks in flight between the element-wise warps and the tensor pipe.  The hand-over of a chunk
+// (pieces stored -> mbarrier -> MMAs issued and executed -> commit -> mbarrier -> piece columns free) is a chain of
+// fixed latencies that two chunks in flight do not cover: the tensor pipe sat idle half of the time.  Here the
+// iteration is split, every kernel has TMEM to spare, and NG = 4 groups of element-wise warps keep four chunks in
+// flight (NG = 2 where KP > 80 leaves no room):
 //
-//   k_tc_h<KS>  H half-step (a1-a5).  TMEM lane = pixel.  No W-phase accumulators, so the BF16 pieces of the H
-//               tile live in TMEM (all three when they fit, else pieces 1 and 2 with piece 3 in shared memory) and
-//               the S stage reads its A operand from TMEM: it runs at the tensor rate and stops competing for the
-//               shared-memory port.  Num/Den take 2 KP columns, so KP = 16 KS goes up to 128 components.
-//               W (3 BF16 pieces, [frames][comps]) is resident in shared memory as in the fused kernel.
-//   k_tc_w<KS>  W half-step (a6-a7) with the new H.  TMEM lane = frame.  One 128-frame M tile per CTA
-//               (blockIdx.z), so a CTA keeps 2 KP accumulator columns (<= 256) and its M tile's rows of W stay in
-//               TMEM for the whole launch (pieces 1, 2; piece 3 in shared memory when KP > 80).  X and Omega rows
-//               are read only by the CTAs of their M tile.  Also the projection kernel (a9) with X = targets,
-//               Omega = omega, W = coef.
+//   k_tc_h<KS,NG>  H half-step (a1-a5).  TMEM lane = pixel.  The BF16 pieces of the H tile live in TMEM (as many of
+//               the three as fit, the others in shared memory), so the S stage reads its A operand from TMEM and
+//               runs at the tensor rate.  Num/Den take 2 KP columns, so KP = 16 KS goes up to 128 components.
+//               W (3 BF16 pieces, [frames][comps]) is resident in shared memory.  The next tile's H pieces are
+//               written as soon as the last S of a tile has completed, before the H update of that tile.
+//   k_tc_w<KS,NG>  W half-step (a6-a7) with the new H.  TMEM lane = frame.  One 128-frame M tile per CTA
+//               (blockIdx.z), so a CTA keeps 2 KP accumulator columns and its M tile's rows of W stay in TMEM for
+//               the whole launch.  The H tile pieces are double-buffered in shared memory when they fit.  X and
+//               Omega rows are read only by the CTAs of their M tile.  Also the projection kernel (a9) with
+//               X = targets, Omega = omega, W = coef.
 //   k_w_update_split   fixed-order fp64 reduction of the per-CTA slabs + W <- W o A / max(B, eps)  (a8)
 //
-// X and Omega cross HBM twice per iteration instead of once (the fused kernel re-reads them through L2), which
-// the roofline of this path accounts for: it is chosen where it is faster (K > 64 always: the fused kernel does
-// not exist there; K <= 64 per measurement, see nmf_tcsplit_prefer()).
-// Arithmetic, operand layouts, ring and barrier protocol are those of nmf_tcfit.cu (BF16x3 split, six piece
-// products per product, FP32 accumulation in TMEM, R1 / R2 written back over S in place).
+// X and Omega cross HBM twice per iteration instead of once (the fused kernel re-reads them through L2).
+// Arithmetic and operand layouts are those of nmf_tcfit.cu (BF16x3 split, six piece products per product, FP32
+// accumulation in TMEM, R1 / R2 written back over S in place).
 #include <cuda.h>
 #include "nmf_common.cuh"
 #include "nmf_tc.cuh"
@@ -28,37 +30,40 @@
 namespace {
 using namespace tc;
 
-constexpr int EW_WARPS = 8;               // two groups of four (one thread per TMEM lane in each group)
-constexpr int W_MMA = 8, W_TMA = 9;
-constexpr int THREADS = 320;
 constexpr int TILE = 128;                 // pixels per tile
 constexpr int FCH = 16;                   // frames per H-step chunk (one UMMA K step)
 constexpr int PCH = 16;                   // pixels per W-step chunk
-constexpr int NCH2 = TILE / PCH;
 constexpr int HS_SB = 16 * 128;           // [128 rows][comps] piece buffers: bytes between 8-component groups
-constexpr int SLOT = 16384;               // ring slot bytes (k_tc_h)
-constexpr int PSW = 32;                   // k_tc_w: pixels per ring slot = one super-chunk (two W-step chunks)
-constexpr int NSW = TILE / PSW;           // k_tc_w: X / Omega slots per tile
-constexpr int SLOTW = 32768;              // k_tc_w ring slot bytes: [64 comps][128 px] of H, or [128 frames][32 px] of X and of Omega
-constexpr int MAX_SLOTS = 8;
+constexpr int SLOT = 16384;               // k_tc_h ring slot: [16 frames][128 px] of X and of Omega, or [16 comps][128 px] of H
+constexpr int PSW = 32;                   // k_tc_w: pixels per X / Omega ring slot (two W-step chunks)
+constexpr int SLOTW = 32768;              // k_tc_w ring slot: [128 frames][32 px] of X and of Omega, or [32 comps][128 px] of H
+constexpr int MAX_SLOTS = 10;
+constexpr int MAX_NG = 4;
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 struct SplitArgs {
-    CUtensorMap mH;            // H   [B*K, P]  box [32 comps][128 px] (k_tc_h) or [64 comps][128 px] (k_tc_w)
+    CUtensorMap mH;            // H   [B*K, P]  box [16 comps][128 px] (k_tc_h) or [32 comps][128 px] (k_tc_w)
     CUtensorMap mX, mO;        // X, Om [B*rows, P]: box [16 frames][128 px] (k_tc_h) or [128 frames][32 px], 128-byte swizzle
                                // (k_tc_w: full 128-byte lines from HBM; 64-byte rows ran the kernel at a quarter of the HBM rate)
     const float* W; float* H; float* slab;
     int N, K; long long P; long long n_tiles;
     int NF;                    // frames padded to a multiple of 16
     int NC;                    // H-step chunks = NF / 16
-    int KH;                    // TMA slots of the H tile (32 components each in k_tc_h, 64 in k_tc_w)
     int NS;                    // ring slots
+    int HB;                    // k_tc_w: buffers of the H tile pieces in shared memory (1 or 2)
 };
 
-enum { B_HS = 0, B_S0, B_S1, B_P0, B_P1, B_G0, B_G1, B_DONE, B_FULL, B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
+enum { B_HS = 0, B_UPD, B_S0, B_S1, B_DONE, B_P0, B_G0 = B_P0 + MAX_NG, B_FULL = B_G0 + MAX_NG,
+       B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
 
 // piece pairs (a, b) of a product, small products first: a1b3 a3b1 a2b2 a1b2 a2b1 a1b1
 __device__ constexpr int PA[6] = {0, 2, 1, 0, 1, 0}, PB[6] = {2, 0, 1, 1, 0, 0};
+
+// pieces of the TMEM-resident A operand of the S stage that fit beside `fixed` columns and NG groups' S / E columns
+__host__ __device__ constexpr int npt_of(int KP, int NG, int fixed) {
+    const int room = 512 - fixed - 64 * NG;
+    return room >= 3 * KP / 2 ? 3 : room >= KP ? 2 : room >= KP / 2 ? 1 : 0;
+}
 
 struct RingCtl {                          // ring slot arithmetic shared by producer and consumers
     uint32_t NS, magic;
@@ -69,47 +74,51 @@ struct RingCtl {                          // ring slot arithmetic shared by prod
     }
 };
 
-// 32 components (rows of a [32][128] fp32 ring slot) of pixel / frame `t` -> three words arrays of 16 (BF16 pairs)
-__device__ __forceinline__ void split_slot32(const float* sl, int t, int k_base, int K, uint32_t (&p1)[16], uint32_t (&p2)[16],
-                                             uint32_t (&p3)[16]) {
-#pragma unroll
-    for (int j = 0; j < 16; ++j) {
-        const int k0 = k_base + 2 * j;
-        const float h0 = k0 < K ? sl[(2 * j) * TILE + t] : 0.f;       // pixels >= P arrive zero-filled
-        const float h1 = k0 + 1 < K ? sl[(2 * j + 1) * TILE + t] : 0.f;
-        split3_pair(h0, h1, p1[j], p2[j], p3[j]);
-    }
-}
 __device__ __forceinline__ void st_piece_smem(unsigned char* base, int t, int kg, const uint32_t* w) {
     *reinterpret_cast<uint4*>(base + (t & 7) * 16 + (t >> 3) * 128 + kg * HS_SB) = make_uint4(w[0], w[1], w[2], w[3]);
 }
-// 32 components' worth of one piece (16 words) into TMEM columns col .. col + 15 of this thread's lane; `ncol` (16 or
-// 8) columns exist (the last 32-component slot is half used when KP % 32 == 16)
-__device__ __forceinline__ void st_piece_tmem(uint32_t taddr, const uint32_t (&w)[16], int ncol) {
-    if (ncol >= 16) tmem_st16(taddr, w);
-    else { const uint32_t h[8] = {w[0], w[1], w[2], w[3], w[4], w[5], w[6], w[7]}; tmem_st8(taddr, h); }
+// 16 components (rows of a ring slot, 128 floats apart) of pixel `t`, components kb .. kb + 15 -> three arrays of 8
+// words; rows at or beyond K hold another problem's data (batched H) or zeros: they are replaced by zeros
+__device__ __forceinline__ void split_rows16(const float* sl, int kb, int K, float* keep, uint32_t (&p1)[8], uint32_t (&p2)[8],
+                                             uint32_t (&p3)[8]) {
+    float h[16];
+#pragma unroll
+    for (int j = 0; j < 16; ++j) h[j] = sl[j * TILE];                         // pixels >= P arrive zero-filled
+    if (kb + 16 > K) {                                                        // rare: the last, partly filled block
+#pragma unroll
+        for (int j = 0; j < 16; ++j) if (kb + j >= K) h[j] = 0.f;
+    }
+#pragma unroll
+    for (int j = 0; j < 8; ++j) {
+        if (keep) { keep[2 * j] = h[2 * j]; keep[2 * j + 1] = h[2 * j + 1]; }
+        split3_pair(h[2 * j], h[2 * j + 1], p1[j], p2[j], p3[j]);
+    }
 }
 
 // =====================================================================================================================
 // H half-step
 // =====================================================================================================================
-template <int KS>
-__global__ void __launch_bounds__(THREADS, 1)
+template <int KS, int NG>
+__global__ void __launch_bounds__(32 * (4 * NG + 2), 1)
 k_tc_h(const __grid_constant__ SplitArgs g) {
     constexpr int KP = 16 * KS;
-    constexpr int NPT = (2 * KP + 3 * KP / 2 + 128 <= 512) ? 3 : 2;       // H pieces kept in TMEM
+    constexpr int EW_WARPS = 4 * NG, W_MMA = EW_WARPS, W_TMA = EW_WARPS + 1, THREADS = 32 * (EW_WARPS + 2);
+    constexpr int NPT = npt_of(KP, NG, 2 * KP);                           // H pieces kept in TMEM
     constexpr uint32_t T_NUM = 0, T_DEN = KP, T_HT = 2 * KP;              // piece i of the H tile at T_HT + i KP / 2
-    constexpr uint32_t T_Z = 2 * KP + NPT * KP / 2, T_E = T_Z + 64;       // Z[jb] at T_Z + 32 jb, E[g] at T_E + 32 g
-    static_assert(T_E + 64 <= 512, "TMEM");
+    constexpr uint32_t T_Z = 2 * KP + NPT * KP / 2, T_E = T_Z + 32 * NG;  // Z[jb] at T_Z + 16 NG jb, E[g] at T_E + 32 g
+    static_assert(T_E + 32 * NG <= 512, "TMEM");
+    constexpr int NBLK = KP / 16;                        // 16-component blocks = H slots per tile
+    constexpr int NB = (NBLK + NG - 1) / NG;             // blocks per group
+    constexpr int HS_BYTES = (KP / 8) * HS_SB;           // one BF16 piece of the H tile in shared memory
     extern __shared__ __align__(1024) unsigned char smem[];
-    const int N = g.N, K = g.K, NF = g.NF, NC = g.NC, KH = g.KH;
+    const int N = g.N, K = g.K, NF = g.NF, NC = g.NC;
     const long long P = g.P;
     const int WS_SB = (NF / 8) * 128;                   // Ws: bytes between 8-component groups
     const int WS_BYTES = (KP / 8) * WS_SB;
     unsigned char* ring = smem;                         // NS slots of 16 KB
     unsigned char* ws_p = ring + (size_t)g.NS * SLOT;   // 3 pieces of W
-    unsigned char* hs3_p = ws_p + 3 * WS_BYTES;         // piece 3 of the H tile (NPT == 2 only)
-    uint64_t* bars = reinterpret_cast<uint64_t*>(hs3_p + (NPT == 2 ? (KP / 8) * HS_SB : 0));
+    unsigned char* hsx_p = ws_p + 3 * WS_BYTES;         // pieces NPT .. 2 of the H tile (those not in TMEM)
+    uint64_t* bars = reinterpret_cast<uint64_t*>(hsx_p + (3 - NPT) * HS_BYTES);
     uint32_t* tptr = reinterpret_cast<uint32_t*>(bars + B_COUNT);
     const RingCtl rc{(uint32_t)g.NS, 0xffffffffu / (uint32_t)g.NS + 1u};
 
@@ -120,9 +129,9 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
     float* __restrict__ H = g.H + (size_t)b * K * P;
 
     if (tid == 0) {
-        mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1);
-        mbar_init(&bars[B_P0], 4); mbar_init(&bars[B_P1], 4); mbar_init(&bars[B_G0], 1); mbar_init(&bars[B_G1], 1);
-        mbar_init(&bars[B_DONE], 1);
+        mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_UPD], EW_WARPS);
+        mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1); mbar_init(&bars[B_DONE], 1);
+        for (int i = 0; i < NG; ++i) { mbar_init(&bars[B_P0 + i], 4); mbar_init(&bars[B_G0 + i], 1); }
         for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 4); }
         mbar_fence_init();
     }
@@ -148,30 +157,41 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tptr;
-    const uint32_t ws_s = smem_u32(ws_p), hs3_s = smem_u32(hs3_p), ring_s = smem_u32(ring);
-    const uint32_t slots_per_tile = (uint32_t)(KH + NC);
-    const int NSC = (NC + 1) / 2;                        // super-chunks of 32 frames (the last may hold 16)
+    const uint32_t ws_s = smem_u32(ws_p), hsx_s = smem_u32(hsx_p), ring_s = smem_u32(ring);
+    const uint32_t slots_per_tile = (uint32_t)(NBLK + NC);
+    const int NSC = (NC + NG - 1) / NG;                  // super-chunks of 16 NG frames (the last may hold fewer)
 
     if (warp == W_TMA) {
         // =========================== TMA producer ===========================
         if (lane == 0) {
             uint32_t seq = 0;
-            auto acquire = [&]() -> uint32_t {            // next ring slot, armed for one full slot
+            auto acquire = [&](uint32_t bytes) -> uint32_t {      // next ring slot, armed for `bytes`
                 uint32_t par;
                 const uint32_t s = rc.slot(seq, par);
                 mbar_wait(&bars[B_EMPTY + s], par ^ 1u);
-                mbar_expect_tx(&bars[B_FULL + s], SLOT);
+                mbar_expect_tx(&bars[B_FULL + s], bytes);
                 ++seq;
                 return s;
             };
+            // L2 prefetch of a whole tile's boxes (H blocks, X and Omega chunks), one tile ahead of the ring loads
+            auto prefetch_tile = [&](long long tile) {
+                if (tile >= g.n_tiles) return;
+                const int p0 = (int)(tile * TILE);
+                for (int h = 0; h < NBLK; ++h) tma_prefetch_l2_2d(&g.mH, p0, b * K + 16 * h);
+                for (int c = 0; c < NC; ++c) {
+                    tma_prefetch_l2_2d(&g.mX, p0, b * N + FCH * c);
+                    tma_prefetch_l2_2d(&g.mO, p0, b * N + FCH * c);
+                }
+            };
             for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
                 const int p0 = (int)(tile * TILE);
-                for (int h = 0; h < KH; ++h) {
-                    const uint32_t s = acquire();
-                    tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
+                prefetch_tile(tile + gridDim.x);
+                for (int h = 0; h < NBLK; ++h) {
+                    const uint32_t s = acquire(16 * TILE * 4);
+                    tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 16 * h, &bars[B_FULL + s]);
                 }
                 for (int c = 0; c < NC; ++c) {
-                    const uint32_t s = acquire();
+                    const uint32_t s = acquire(2 * FCH * TILE * 4);
                     tma_load_2d(ring_s + s * SLOT, &g.mX, p0, b * N + FCH * c, &bars[B_FULL + s]);
                     tma_load_2d(ring_s + s * SLOT + FCH * TILE * 4, &g.mO, p0, b * N + FCH * c, &bars[B_FULL + s]);
                 }
@@ -181,29 +201,31 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
         // =========================== MMA issuer (whole warp converged; one elected lane issues) ===========================
         uint32_t ph = 0;
         auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; tc_fence_after(); };
-        constexpr uint32_t id_s32 = idesc_bf16(128, 32, 0), id_s16 = idesc_bf16(128, 16, 0), id_nd = idesc_bf16(128, KP, 1);
-        uint64_t d_ws_k[3], d_ws_mn[3];
+        constexpr uint32_t id_nd = idesc_bf16(128, KP, 1);
+        uint64_t d_ws_k[3], d_ws_mn[3], d_hsx_k[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             d_ws_k[i] = smem_desc(ws_s + i * WS_BYTES, WS_SB, 128);
             d_ws_mn[i] = smem_desc(ws_s + i * WS_BYTES, 128, WS_SB);
+            d_hsx_k[i] = smem_desc(hsx_s + (i >= NPT ? i - NPT : 0) * HS_BYTES, HS_SB, 128);
         }
-        const uint64_t d_hs3_k = smem_desc(hs3_s, HS_SB, 128);
         const uint32_t ws_kstep = (uint32_t)(2 * WS_SB) >> 4;
         constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
+        bool first = true;
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
-            auto issue_S = [&](int j) {                  // S(j): [128 px] x [32 frames], K = comps -> Z[j & 1]
+            auto issue_S = [&](int j) {                  // S(j): [128 px] x [16 NG frames], K = comps -> Z[j & 1]
                 if (elect_one()) {
-                    const uint32_t d = tmem + T_Z + 32 * (j & 1);
-                    const uint32_t boff = (uint32_t)(j * 4 * 128) >> 4;
-                    const uint32_t id = (2 * j + 1 < NC) ? id_s32 : id_s16;
+                    const uint32_t d = tmem + T_Z + 16 * NG * (j & 1);
+                    const uint32_t boff = (uint32_t)(j * NG * 2 * 128) >> 4;      // 16 frames = 2 row groups of 128 bytes
+                    const int nch = NC - NG * j < NG ? NC - NG * j : NG;
+                    const uint32_t id = idesc_bf16(128, 16 * nch, 0);
 #pragma unroll
                     for (int pr = 0; pr < 6; ++pr)
 #pragma unroll
                         for (int ks = 0; ks < KS; ++ks) {
                             const uint64_t bd = d_ws_k[PB[pr]] + boff + ks * ws_kstep;
                             if (PA[pr] < NPT) mma16_ts(d, tmem + T_HT + PA[pr] * (KP / 2) + 8 * ks, bd, id, (pr | ks) ? 1u : 0u);
-                            else mma16_ss(d, d_hs3_k + ks * hs_kstep, bd, id, (pr | ks) ? 1u : 0u);
+                            else mma16_ss(d, d_hsx_k[PA[pr]] + ks * hs_kstep, bd, id, (pr | ks) ? 1u : 0u);
                         }
                     mma_commit(&bars[B_S0 + (j & 1)]);
                 }
@@ -212,13 +234,15 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             wait(B_HS);
             issue_S(0);
             if (NSC > 1) issue_S(1);
+            if (!first) wait(B_UPD);                     // the previous tile's update has read Num / Den
+            first = false;
             for (int j = 0; j < NSC; ++j) {
-                for (int gg = 0; gg < 2; ++gg) {
-                    const int c = 2 * j + gg;
+                for (int gg = 0; gg < NG; ++gg) {
+                    const int c = NG * j + gg;
                     if (c >= NC) break;
                     wait(B_P0 + gg);
                     if (elect_one()) {
-                        const uint32_t z = tmem + T_Z + 32 * (j & 1) + 16 * gg, e = tmem + T_E + 32 * gg;
+                        const uint32_t z = tmem + T_Z + 16 * NG * (j & 1) + 16 * gg, e = tmem + T_E + 32 * gg;
                         const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
                         const uint32_t a_r[3] = {z, z + 8, e + O_R3};
                         const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 frames = 2 row groups
@@ -238,7 +262,7 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             __syncwarp();
         }
     } else if (warp < EW_WARPS) {
-        // =========================== element-wise warps ===========================
+        // =========================== element-wise warps: group grp = warp / 4, lane quadrant q = warp % 4 ===========================
         const int q = warp & 3, grp = warp >> 2;
         const int t = 32 * q + lane;                     // TMEM lane = pixel of the tile
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
@@ -259,92 +283,113 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[bar]);
         };
-        uint32_t sq = 0;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
-            const long long p = tile * TILE + t;
-            const bool p_ok = p < P;
-            const long long pc = p_ok ? p : P - 1;
-
-            // ---- H0: the H tile's pieces -> TMEM (A operand of S); group g takes the 32-component slots g, g + 2, ...
-            // (every MMA of the previous tile is complete: this warp waited for B_DONE in its update step)
-            for (int h = grp; h < KH; h += 2) {
-                const float* hsl = reinterpret_cast<const float*>(wait_full(sq + h));
-                uint32_t p1[16], p2[16], p3[16];
-                split_slot32(hsl, t, 32 * h, K, p1, p2, p3);
-                release(sq + h);
-                const int ncol = KP / 2 - 16 * h;        // columns of this slot that exist (16, or 8 in a half-used last slot)
-                if (ncol > 0) {
-                    st_piece_tmem(lane_base + T_HT + 16 * h, p1, ncol);
-                    st_piece_tmem(lane_base + T_HT + KP / 2 + 16 * h, p2, ncol);
-                    if (NPT == 3) st_piece_tmem(lane_base + T_HT + KP + 16 * h, p3, ncol);
-                    else {
+        // H0: the pieces of a tile's H -> TMEM / shared memory (A operand of S); group g takes the 16-component blocks
+        // g, g + NG, ... (one ring slot each) and keeps their fp32 values for the update
+        auto h0 = [&](uint32_t sqt, float (&hv)[NB][16]) {
 #pragma unroll
-                        for (int gq = 0; gq < 4; ++gq)
-                            if (4 * h + gq < KP / 8) st_piece_smem(hs3_p, t, 4 * h + gq, &p3[4 * gq]);
+            for (int bb = 0; bb < NB; ++bb) {
+                const int bi = grp + NG * bb;
+                if (bi < NBLK) {
+                    const float* hsl = reinterpret_cast<const float*>(wait_full(sqt + bi)) + t;
+                    uint32_t p[3][8];
+                    split_rows16(hsl, 16 * bi, K, hv[bb], p[0], p[1], p[2]);
+                    release(sqt + bi);
+#pragma unroll
+                    for (int i = 0; i < 3; ++i) {
+                        if (i < NPT) tmem_st8(lane_base + T_HT + i * (KP / 2) + 8 * bi, p[i]);
+                        else {
+                            st_piece_smem(hsx_p + (i - NPT) * HS_BYTES, t, 2 * bi, &p[i][0]);
+                            st_piece_smem(hsx_p + (i - NPT) * HS_BYTES, t, 2 * bi + 1, &p[i][4]);
+                        }
                     }
                 }
             }
             tmem_wait_st();
-            if (NPT == 2) fence_proxy_async();
+            if (NPT < 3) fence_proxy_async();
             tc_fence_before();
             warp_arrive(B_HS);
-
-            // ---- steps: super-chunk j = chunks 2j (group 0) and 2j + 1 (group 1); thread = (pixel t, 16 frames) ----
+        };
+        float hold[NB][16];
+        uint32_t sq = 0;
+        h0(0, hold);
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
+            // ---- steps: super-chunk j = chunks NG j + grp; thread = (pixel t, 16 frames), two halves of 8 ----
             bool pending = false;
             for (int j = 0; j < NSC; ++j) {
-                const int c = 2 * j + grp;
+                const int c = NG * j + grp;
                 const bool have = c < NC;
-                float x[16], o[16];
-                if (have) {
-                    const float* xs = reinterpret_cast<const float*>(wait_full(sq + KH + c)) + t;
-                    const int nv = N - FCH * c;          // valid frames of this chunk (>= 16: all)
-#pragma unroll
-                    for (int i = 0; i < 16; ++i) {
-                        x[i] = xs[i * TILE];
-                        o[i] = i < nv ? xs[FCH * TILE + i * TILE] : 0.f;
-                    }
-                }
-                wait(B_S0 + (j & 1));                    // both groups track every completion of the buffer's barrier
+                const float* xs = nullptr;
+                if (have) xs = reinterpret_cast<const float*>(wait_full(sq + NBLK + c)) + t;
+                wait(B_S0 + (j & 1));                    // every group tracks every completion of the buffer's barrier
                 if (have) {
                     tc_fence_after();
-                    const uint32_t zcol = lane_base + T_Z + 32 * (j & 1) + 16 * grp;
-                    uint32_t s[16], e[32];
+                    const uint32_t zcol = lane_base + T_Z + 16 * NG * (j & 1) + 16 * grp;
+                    const uint32_t ecol = lane_base + T_E + 32 * grp;
+                    const int nv = N - FCH * c;          // valid frames of this chunk (>= 16: all)
+                    uint32_t s[16];
                     tmem_ld16(zcol, s);
                     tmem_wait_ld();
-                    ew16(x, o, s, zcol, e);
-                    release(sq + KH + c);                // after the values were consumed
-                    if (pending) { wait(B_G0 + grp); tc_fence_after(); }
-                    tmem_st32(lane_base + T_E + 32 * grp, e);
+                    if (pending) { wait(B_G0 + grp); tc_fence_after(); }      // this group's E columns are free again
+#pragma unroll
+                    for (int hf = 0; hf < 2; ++hf) {
+                        float x[8], o[8];
+#pragma unroll
+                        for (int i = 0; i < 8; ++i) {
+                            x[i] = xs[(8 * hf + i) * TILE];
+                            o[i] = xs[FCH * TILE + (8 * hf + i) * TILE];
+                        }
+                        if (nv < 16) {                   // rare: frames past N (another problem's rows in a batch)
+#pragma unroll
+                            for (int i = 0; i < 8; ++i) if (8 * hf + i >= nv) o[i] = 0.f;
+                        }
+                        Ew8 w;
+                        ew8(x, o, &s[8 * hf], w);
+                        ew8_store(zcol, ecol, hf, w);
+                    }
+                    release(sq + NBLK + c);              // after the values were consumed
                     tmem_wait_st();
                     tc_fence_before();
                     warp_arrive(B_P0 + grp);
                     pending = true;
                 }
             }
-            // ---- update: h' = h * num / max(den, eps) in place; thread = (pixel t, this group's half of the comps);
-            // the old h is re-read from global memory (it was loaded by TMA a moment ago: L2) ----
+            // ---- every S of this tile has completed (each warp waited for all of them): the next tile's H pieces ----
+            // (only where a thread keeps one block of 16 values: two live sets of NB x 16 registers would spill)
+            constexpr bool EARLY = NB == 1;
+            float hnext[NB][16];
+            const bool has_next = tile + gridDim.x < g.n_tiles;
+            if constexpr (EARLY) { if (has_next) h0(sq + slots_per_tile, hnext); }
+            // ---- update: h' = h * num / max(den, eps) in place; thread = (pixel t, the components it split in H0) ----
             if (pending) wait(B_G0 + grp);
-            wait(B_DONE);                                // Num, Den complete; every S has read the H pieces
+            wait(B_DONE);                                // Num, Den complete
             tc_fence_after();
-            {
-                constexpr int NKG = KP / 8;              // 8-component groups; group g updates NKG / 2 of them
-                for (int kg = grp * (NKG / 2); kg < (grp + 1) * (NKG / 2); ++kg) {
-                    float* hp = H + (size_t)(8 * kg) * P + pc;
-                    float hold[8];
+            const long long p = tile * TILE + t;
+            const bool p_ok = p < P;
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) hold[j] = (8 * kg + j < K) ? hp[(size_t)j * P] : 0.f;
-                    uint32_t nm[8], dn[8];
-                    tmem_ld8(lane_base + T_NUM + 8 * kg, nm);
-                    tmem_ld8(lane_base + T_DEN + 8 * kg, dn);
+            for (int bb = 0; bb < NB; ++bb) {
+                const int kb = 16 * (grp + NG * bb);
+                if (kb < KP) {                           // (warp-uniform: tcgen05.ld is warp-collective)
+                    uint32_t nm[16], dn[16];
+                    tmem_ld16(lane_base + T_NUM + kb, nm);
+                    tmem_ld16(lane_base + T_DEN + kb, dn);
                     tmem_wait_ld();
+                    float* hp = H + (size_t)kb * P + (p_ok ? p : 0);
+                    const int kv = p_ok ? K - kb : 0;    // components of this block that exist (none for a pixel past P)
 #pragma unroll
-                    for (int j = 0; j < 8; ++j) {
-                        const float v = __fdividef(hold[j] * __uint_as_float(nm[j]), fmaxf(__uint_as_float(dn[j]), NMF_EPS));
-                        if (p_ok && 8 * kg + j < K) hp[(size_t)j * P] = v;
+                    for (int j = 0; j < 16; ++j, hp += P) {
+                        const float v = __fdividef(hold[bb][j] * __uint_as_float(nm[j]), fmaxf(__uint_as_float(dn[j]), NMF_EPS));
+                        if (j < kv) *hp = v;
                     }
                 }
             }
             tc_fence_before();
+            warp_arrive(B_UPD);
+            if (has_next) {
+                if constexpr (EARLY) {
+#pragma unroll
+                    for (int j = 0; j < 16; ++j) hold[0][j] = hnext[0][j];
+                } else h0(sq + slots_per_tile, hold);
+            }
         }
     }
     tc_fence_before();
@@ -355,23 +400,27 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
 // =====================================================================================================================
 // W half-step (and projection)
 // =====================================================================================================================
-template <int KS>
-__global__ void __launch_bounds__(THREADS, 1)
+template <int KS, int NG>
+__global__ void __launch_bounds__(32 * (4 * NG + 2), 1)
 k_tc_w(const __grid_constant__ SplitArgs g) {
     constexpr int KP = 16 * KS;
-    constexpr int NPT = (3 * KP / 2 + 128 <= 256) ? 3 : 2;                // W pieces of the M tile kept in TMEM
+    constexpr int EW_WARPS = 4 * NG, W_MMA = EW_WARPS, W_TMA = EW_WARPS + 1;
+    constexpr int NPT = npt_of(KP, NG, 2 * KP);                           // W pieces of the M tile kept in TMEM
     constexpr uint32_t T_WT = 0;                                          // piece i at i KP / 2
-    constexpr uint32_t T_Z = NPT * KP / 2, T_E = T_Z + 64;                // Z[jb] at T_Z + 32 jb, E[g] at T_E + 32 g
-    constexpr uint32_t T_ACC = 256;                                       // A at T_ACC, B at T_ACC + KP
-    static_assert(T_E + 64 <= 256 && T_ACC + 2 * KP <= 512, "TMEM");
+    constexpr uint32_t T_Z = NPT * KP / 2, T_E = T_Z + 32 * NG;           // Z[jb] at T_Z + 16 NG jb, E[g] at T_E + 32 g
+    constexpr uint32_t T_ACC = 512 - 2 * KP;                              // A at T_ACC, B at T_ACC + KP
+    static_assert(T_E + 32 * NG <= T_ACC, "TMEM");
+    constexpr int NBLK = KP / 16;                        // 16-component blocks
+    constexpr int NHS = (NBLK + 1) / 2;                  // H ring slots (32 components each) per tile
+    constexpr int NSW = TILE / PSW;                      // X / Omega ring slots per tile
+    constexpr int NSC2 = TILE / (PCH * NG);              // super-chunks of 16 NG pixels per tile
+    constexpr int HS_BYTES = (KP / 8) * HS_SB;           // one BF16 piece of the H tile / of the M tile's W rows
     extern __shared__ __align__(1024) unsigned char smem[];
-    const int N = g.N, K = g.K, KH = g.KH;
-    const long long P = g.P;
-    constexpr int HS_BYTES = (KP / 8) * HS_SB;          // one BF16 piece of the H tile / of the M tile's W rows
+    const int N = g.N, K = g.K, HB = g.HB;
     unsigned char* ring = smem;
-    unsigned char* hs_p = ring + (size_t)g.NS * SLOTW;  // 3 pieces of the H tile, [pixel][comp]
-    unsigned char* ws3_p = hs_p + 3 * HS_BYTES;         // piece 3 of this M tile's rows of W (NPT == 2 only)
-    uint64_t* bars = reinterpret_cast<uint64_t*>(ws3_p + (NPT == 2 ? HS_BYTES : 0));
+    unsigned char* hs_p = ring + (size_t)g.NS * SLOTW;  // HB x 3 pieces of the H tile, [pixel][comp]
+    unsigned char* wsx_p = hs_p + (size_t)HB * 3 * HS_BYTES;     // pieces NPT .. 2 of this M tile's rows of W
+    uint64_t* bars = reinterpret_cast<uint64_t*>(wsx_p + (3 - NPT) * HS_BYTES);
     uint32_t* tptr = reinterpret_cast<uint32_t*>(bars + B_COUNT);
     const RingCtl rc{(uint32_t)g.NS, 0xffffffffu / (uint32_t)g.NS + 1u};
 
@@ -383,10 +432,10 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     float* slab = g.slab + (((size_t)b * gridDim.z + m) * gridDim.x + blockIdx.x) * 2 * (size_t)128 * KP;
 
     if (tid == 0) {
-        mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1);
-        mbar_init(&bars[B_P0], 4); mbar_init(&bars[B_P1], 4); mbar_init(&bars[B_G0], 1); mbar_init(&bars[B_G1], 1);
-        mbar_init(&bars[B_DONE], 1);
-        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], EW_WARPS); }
+        mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_UPD], 1);     // B_UPD: every MMA of the launch is complete
+        mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1); mbar_init(&bars[B_DONE], 1);
+        for (int i = 0; i < NG; ++i) { mbar_init(&bars[B_P0 + i], 4); mbar_init(&bars[B_G0 + i], 1); }
+        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 8); }
         mbar_fence_init();
     }
     if (warp == W_MMA) tmem_alloc(tptr, 512);
@@ -395,36 +444,35 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     __syncthreads();
     tc_fence_after();
     const uint32_t tmem = *tptr;
-    const uint32_t hs_s = smem_u32(hs_p), ws3_s = smem_u32(ws3_p), ring_s = smem_u32(ring);
-    const uint32_t slots_per_tile = (uint32_t)(KH + NSW);
-    constexpr int NSC2 = NCH2 / 2;
+    const uint32_t hs_s = smem_u32(hs_p), wsx_s = smem_u32(wsx_p), ring_s = smem_u32(ring);
+    const uint32_t slots_per_tile = (uint32_t)(NHS + NSW);
 
     if (warp < EW_WARPS) {
-        // the M tile's rows of W -> TMEM (A operand of S', fixed for the launch); lane = frame 128 m + t
+        // the M tile's rows of W -> TMEM / shared memory (A operand of S', fixed for the launch); lane = frame 128 m + t;
+        // group g takes the 16-component blocks g, g + NG, ...
         const int q = warp & 3, grp = warp >> 2, t = 32 * q + lane;
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
         const int fr = 128 * m + t;
-        for (int h = grp; 32 * h < KP; h += 2) {
-            uint32_t p1[16], p2[16], p3[16];
+        for (int bi = grp; bi < NBLK; bi += NG) {
+            uint32_t p[3][8];
 #pragma unroll
-            for (int j = 0; j < 16; ++j) {
-                const int k0 = 32 * h + 2 * j;
+            for (int j = 0; j < 8; ++j) {
+                const int k0 = 16 * bi + 2 * j;
                 const float w0 = (fr < N && k0 < K) ? W[(size_t)fr * K + k0] : 0.f;
                 const float w1 = (fr < N && k0 + 1 < K) ? W[(size_t)fr * K + k0 + 1] : 0.f;
-                split3_pair(w0, w1, p1[j], p2[j], p3[j]);
+                split3_pair(w0, w1, p[0][j], p[1][j], p[2][j]);
             }
-            const int ncol = KP / 2 - 16 * h;
-            st_piece_tmem(lane_base + T_WT + 16 * h, p1, ncol);
-            st_piece_tmem(lane_base + T_WT + KP / 2 + 16 * h, p2, ncol);
-            if (NPT == 3) st_piece_tmem(lane_base + T_WT + KP + 16 * h, p3, ncol);
-            else {
 #pragma unroll
-                for (int gq = 0; gq < 4; ++gq)
-                    if (4 * h + gq < KP / 8) st_piece_smem(ws3_p, t, 4 * h + gq, &p3[4 * gq]);
+            for (int i = 0; i < 3; ++i) {
+                if (i < NPT) tmem_st8(lane_base + T_WT + i * (KP / 2) + 8 * bi, p[i]);
+                else {
+                    st_piece_smem(wsx_p + (i - NPT) * HS_BYTES, t, 2 * bi, &p[i][0]);
+                    st_piece_smem(wsx_p + (i - NPT) * HS_BYTES, t, 2 * bi + 1, &p[i][4]);
+                }
             }
         }
         tmem_wait_st();
-        if (NPT == 2) fence_proxy_async();
+        if (NPT < 3) fence_proxy_async();
         tc_fence_before();
     }
     __syncthreads();
@@ -434,22 +482,33 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
         // =========================== TMA producer ===========================
         if (lane == 0) {
             uint32_t seq = 0;
-            auto acquire = [&]() -> uint32_t {
+            auto acquire = [&](uint32_t bytes) -> uint32_t {
                 uint32_t par;
                 const uint32_t s = rc.slot(seq, par);
                 mbar_wait(&bars[B_EMPTY + s], par ^ 1u);
-                mbar_expect_tx(&bars[B_FULL + s], SLOTW);
+                mbar_expect_tx(&bars[B_FULL + s], bytes);
                 ++seq;
                 return s;
             };
+            // L2 prefetch of a whole tile's boxes, one tile ahead of the ring loads
+            auto prefetch_tile = [&](long long tile) {
+                if (tile >= g.n_tiles) return;
+                const int p0 = (int)(tile * TILE);
+                for (int h = 0; h < NHS; ++h) tma_prefetch_l2_2d(&g.mH, p0, b * K + 32 * h);
+                for (int c = 0; c < NSW; ++c) {
+                    tma_prefetch_l2_2d(&g.mX, p0 + PSW * c, b * N + 128 * m);
+                    tma_prefetch_l2_2d(&g.mO, p0 + PSW * c, b * N + 128 * m);
+                }
+            };
             for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
                 const int p0 = (int)(tile * TILE);
-                for (int h = 0; h < KH; ++h) {
-                    const uint32_t s = acquire();
-                    tma_load_2d(ring_s + s * SLOTW, &g.mH, p0, b * K + 64 * h, &bars[B_FULL + s]);
+                prefetch_tile(tile + gridDim.x);
+                for (int h = 0; h < NHS; ++h) {
+                    const uint32_t s = acquire(32 * TILE * 4);
+                    tma_load_2d(ring_s + s * SLOTW, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
                 }
-                for (int c = 0; c < NSW; ++c) {          // the M tile's 128 rows of X and Omega, 32 px (one super-chunk) at a time
-                    const uint32_t s = acquire();
+                for (int c = 0; c < NSW; ++c) {          // the M tile's 128 rows of X and Omega, 32 px (two chunks) at a time
+                    const uint32_t s = acquire(SLOTW);
                     tma_load_2d(ring_s + s * SLOTW, &g.mX, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
                     tma_load_2d(ring_s + s * SLOTW + 128 * PSW * 4, &g.mO, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
                 }
@@ -459,43 +518,45 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
         // =========================== MMA issuer ===========================
         uint32_t ph = 0;
         auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; tc_fence_after(); };
-        constexpr uint32_t id_s32 = idesc_bf16(128, 32, 0), id_ab = idesc_bf16(128, KP, 1);
-        uint64_t d_hs_k[3], d_hs_mn[3];
+        constexpr uint32_t id_s = idesc_bf16(128, 16 * NG, 0), id_ab = idesc_bf16(128, KP, 1);
+        uint64_t d_hs_k[3], d_hs_mn[3], d_wsx_k[3];
 #pragma unroll
         for (int i = 0; i < 3; ++i) {
             d_hs_k[i] = smem_desc(hs_s + i * HS_BYTES, HS_SB, 128);
             d_hs_mn[i] = smem_desc(hs_s + i * HS_BYTES, 128, HS_SB);
+            d_wsx_k[i] = smem_desc(wsx_s + (i >= NPT ? i - NPT : 0) * HS_BYTES, HS_SB, 128);
         }
-        const uint64_t d_ws3_k = smem_desc(ws3_s, HS_SB, 128);
         constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
         bool acc_started = false;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
-            auto issue_S2 = [&](int j) {                 // S'(j): [128 frames] x [32 px], K = comps -> Z[j & 1]
+        uint32_t it = 0;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, ++it) {
+            const uint32_t hboff = (HB == 2 && (it & 1u)) ? (uint32_t)(3 * HS_BYTES) >> 4 : 0u;      // this tile's Hs buffer
+            auto issue_S2 = [&](int j) {                 // S'(j): [128 frames] x [16 NG px], K = comps -> Z[j & 1]
                 if (elect_one()) {
-                    const uint32_t boff = (uint32_t)(j * 4 * 128) >> 4;
-                    const uint32_t d = tmem + T_Z + 32 * (j & 1);
+                    const uint32_t boff = hboff + ((uint32_t)(j * NG * 2 * 128) >> 4);
+                    const uint32_t d = tmem + T_Z + 16 * NG * (j & 1);
 #pragma unroll
                     for (int pr = 0; pr < 6; ++pr)
 #pragma unroll
                         for (int ks = 0; ks < KS; ++ks) {
                             const uint64_t bd = d_hs_k[PB[pr]] + boff + ks * hs_kstep;
-                            if (PA[pr] < NPT) mma16_ts(d, tmem + T_WT + PA[pr] * (KP / 2) + 8 * ks, bd, id_s32, (pr | ks) ? 1u : 0u);
-                            else mma16_ss(d, d_ws3_k + ks * hs_kstep, bd, id_s32, (pr | ks) ? 1u : 0u);
+                            if (PA[pr] < NPT) mma16_ts(d, tmem + T_WT + PA[pr] * (KP / 2) + 8 * ks, bd, id_s, (pr | ks) ? 1u : 0u);
+                            else mma16_ss(d, d_wsx_k[PA[pr]] + ks * hs_kstep, bd, id_s, (pr | ks) ? 1u : 0u);
                         }
                     mma_commit(&bars[B_S0 + (j & 1)]);
                 }
                 __syncwarp();
             };
-            wait(B_HS);                                  // the new H tile's pieces are in Hs
+            wait(B_HS);                                  // the new H tile's pieces are in this tile's Hs buffer
             issue_S2(0);
-            issue_S2(1);
+            if (NSC2 > 1) issue_S2(1);
             for (int j = 0; j < NSC2; ++j) {
-                for (int gg = 0; gg < 2; ++gg) {
-                    const int c = 2 * j + gg;
+                for (int gg = 0; gg < NG; ++gg) {
+                    const int c = NG * j + gg;
                     wait(B_P0 + gg);
                     if (elect_one()) {
-                        const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
-                        const uint32_t z = tmem + T_Z + 32 * (j & 1) + 16 * gg, e = tmem + T_E + 32 * gg;
+                        const uint32_t boff = hboff + ((uint32_t)(c * 2 * 128) >> 4);   // 16 pixels = 2 row groups
+                        const uint32_t z = tmem + T_Z + 16 * NG * (j & 1) + 16 * gg, e = tmem + T_E + 32 * gg;
                         const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
                         const uint32_t a_r[3] = {z, z + 8, e + O_R3};
 #pragma unroll
@@ -511,11 +572,15 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                 }
                 if (j + 2 < NSC2) issue_S2(j + 2);
             }
-            if (elect_one()) mma_commit(&bars[B_DONE]);
-            __syncwarp();
+            if (HB == 1) {                               // single Hs buffer: the next H0 waits for every MMA of this tile
+                if (elect_one()) mma_commit(&bars[B_DONE]);
+                __syncwarp();
+            }
         }
+        if (elect_one()) mma_commit(&bars[B_UPD]);       // every MMA of the launch is complete
+        __syncwarp();
     } else if (warp < EW_WARPS) {
-        // =========================== element-wise warps ===========================
+        // =========================== element-wise warps: group grp = warp / 4, lane quadrant q = warp % 4 ===========================
         const int q = warp & 3, grp = warp >> 2;
         const int t = 32 * q + lane;                     // TMEM lane = frame 128 m + t
         const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
@@ -538,83 +603,90 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[bar]);
         };
-        uint32_t sq = 0;
-        bool first = true;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
-            // ---- H0: the (new) H tile is split into Hs[pixel][comp]; thread = pixel t; a slot holds 64 components,
-            // group g takes components 64 h + 32 g .. + 31 of slot h
-            if (!first) wait(B_DONE);                    // every MMA of the previous tile is complete: Hs is free
-            first = false;
-            for (int h = 0; h < KH; ++h) {
-                const float* hsl = reinterpret_cast<const float*>(wait_full(sq + h)) + (32 * grp) * TILE;
-                const int hh = 2 * h + grp;              // 32-component block
-                if (32 * hh < KP) {
-                    uint32_t p1[16], p2[16], p3[16];
-                    split_slot32(hsl, t, 32 * hh, K, p1, p2, p3);
+        // H0: the (new) H tile is split into Hs[buffer][pixel][comp]; thread = pixel t.  Ring slot h holds the
+        // components 32 h .. 32 h + 31: its two 16-component blocks go to the groups (2 h) % NG and (2 h + 1) % NG, so
+        // every slot is released by exactly eight warps, like an X / Omega slot.
+        auto h0 = [&](uint32_t sqt, uint32_t buf) {
+            unsigned char* hb = hs_p + (size_t)buf * 3 * HS_BYTES;
+            for (int h = 0; h < NHS; ++h) {
+                const int sub = (grp - 2 * h) & (NG - 1);            // 0 or 1: this group's block of the slot
+                if (sub < 2) {
+                    const int bi = 2 * h + sub;
+                    const float* hsl = reinterpret_cast<const float*>(wait_full(sqt + h)) + (16 * sub) * TILE + t;
+                    if (bi < NBLK) {
+                        uint32_t p[3][8];
+                        split_rows16(hsl, 16 * bi, K, nullptr, p[0], p[1], p[2]);
 #pragma unroll
-                    for (int gq = 0; gq < 4; ++gq)
-                        if (4 * hh + gq < KP / 8) {
-                            st_piece_smem(hs_p, t, 4 * hh + gq, &p1[4 * gq]);
-                            st_piece_smem(hs_p + HS_BYTES, t, 4 * hh + gq, &p2[4 * gq]);
-                            st_piece_smem(hs_p + 2 * HS_BYTES, t, 4 * hh + gq, &p3[4 * gq]);
+                        for (int i = 0; i < 3; ++i) {
+                            st_piece_smem(hb + i * HS_BYTES, t, 2 * bi, &p[i][0]);
+                            st_piece_smem(hb + i * HS_BYTES, t, 2 * bi + 1, &p[i][4]);
                         }
+                    }
+                    release(sqt + h);
                 }
-                release(sq + h);
             }
             fence_proxy_async();
             warp_arrive(B_HS);
-
-            // ---- steps: super-chunk j = chunks 2j + grp; thread = (frame 128 m + t, 16 pixels) ----
+        };
+        uint32_t sq = 0, it = 0;
+        h0(0, 0);
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile, ++it) {
+            // ---- steps: chunk c = NG j + grp of super-chunk j; thread = (frame 128 m + t, 16 pixels), two halves of 8 ----
             bool pending = false;
+            const int sw = t & 7;
             for (int j = 0; j < NSC2; ++j) {
-                const uint32_t seq = sq + KH + j;        // both groups read the super-chunk's slot: group g its pixels 16 g .. 16 g + 15
-                const unsigned char* xsl = wait_full(seq);           // X rows (128 bytes each, 128-byte swizzle) at +0, Omega rows at +16 KB
-                float x[16], o[16];
+                const int c = NG * j + grp;
+                const uint32_t seq = sq + NHS + (c >> 1);            // ring slot of 32 pixels: chunks 2 s and 2 s + 1
+                const unsigned char* xsl = wait_full(seq) + t * 128;     // X rows (128 bytes each, 128-byte swizzle) at +0, Omega rows at +16 KB
+                wait(B_S0 + (j & 1)); tc_fence_after();
+                const uint32_t zcol = lane_base + T_Z + 16 * NG * (j & 1) + 16 * grp;
+                const uint32_t ecol = lane_base + T_E + 32 * grp;
+                uint32_t s[16];
+                if (active) { tmem_ld16(zcol, s); tmem_wait_ld(); }
+                if (pending) { wait(B_G0 + grp); tc_fence_after(); }      // this group's E columns are free again
                 if (active) {
-                    if (fr < N) {
-                        const int sw = t & 7;
 #pragma unroll
-                        for (int ch = 0; ch < 4; ++ch) {
-                            const int cs = ((4 * grp + ch) ^ sw) << 4;
-                            const float4 xv = *reinterpret_cast<const float4*>(xsl + t * 128 + cs);
-                            const float4 ov = *reinterpret_cast<const float4*>(xsl + 128 * PSW * 4 + t * 128 + cs);
+                    for (int hf = 0; hf < 2; ++hf) {
+                        float x[8], o[8];
+#pragma unroll
+                        for (int ch = 0; ch < 2; ++ch) {
+                            float4 xv = make_float4(0.f, 0.f, 0.f, 0.f), ov = xv;
+                            if (fr < N) {
+                                const int cs = ((4 * (c & 1) + 2 * hf + ch) ^ sw) << 4;
+                                xv = *reinterpret_cast<const float4*>(xsl + cs);
+                                ov = *reinterpret_cast<const float4*>(xsl + 128 * PSW * 4 + cs);
+                            }
                             x[4 * ch] = xv.x; x[4 * ch + 1] = xv.y; x[4 * ch + 2] = xv.z; x[4 * ch + 3] = xv.w;
                             o[4 * ch] = ov.x; o[4 * ch + 1] = ov.y; o[4 * ch + 2] = ov.z; o[4 * ch + 3] = ov.w;
                         }
-                    } else {
-#pragma unroll
-                        for (int i = 0; i < 16; ++i) { x[i] = 0.f; o[i] = 0.f; }
+                        Ew8 w;
+                        ew8(x, o, &s[8 * hf], w);
+                        ew8_store(zcol, ecol, hf, w);
                     }
                 }
-                wait(B_S0 + (j & 1)); tc_fence_after();
-                uint32_t e[32];
-                if (active) {
-                    const uint32_t zcol = lane_base + T_Z + 32 * (j & 1) + 16 * grp;
-                    uint32_t s[16];
-                    tmem_ld16(zcol, s);
-                    tmem_wait_ld();
-                    ew16(x, o, s, zcol, e);
-                }
                 release(seq);                            // after the values were consumed
-                if (pending) { wait(B_G0 + grp); tc_fence_after(); }
-                if (active) tmem_st32(lane_base + T_E + 32 * grp, e);
                 tmem_wait_st();
                 tc_fence_before();
                 warp_arrive(B_P0 + grp);
                 pending = true;
             }
-            wait(B_G0 + grp);
+            wait(B_G0 + grp);                            // this group's last AB of the tile is complete, and with it (the
+                                                         // tensor pipe completes in order) every MMA of the previous tile
+            if (tile + gridDim.x < g.n_tiles) {
+                if (HB == 1) wait(B_DONE);               // single buffer: every MMA of this tile must be complete
+                h0(sq + slots_per_tile, HB == 2 ? ((it + 1) & 1u) : 0u);
+            }
         }
-        wait(B_DONE);                                    // every MMA of the last tile is complete
+        wait(B_UPD);                                     // every MMA of the launch is complete
         tc_fence_after();
-        // ---- accumulators -> this CTA's slab [2][128][KP] (grid.x <= n_tiles: every CTA had a tile) ----
-        constexpr int NCG = KP / 16;                     // 16-column groups; group g writes its share
-        for (int cg = grp ? (NCG + 1) / 2 : 0; cg < (grp ? NCG : (NCG + 1) / 2); ++cg) {
+        // ---- accumulators -> this CTA's slab [2][128][KP] (grid.x <= n_tiles: every CTA had a tile); group g writes
+        // the 16-column blocks g, g + NG, ... ----
+        for (int cb = 16 * grp; cb < KP; cb += 16 * NG) {
             uint32_t a[16], bq[16];
-            tmem_ld16(lane_base + T_ACC + 16 * cg, a);
-            tmem_ld16(lane_base + T_ACC + KP + 16 * cg, bq);
+            tmem_ld16(lane_base + T_ACC + cb, a);
+            tmem_ld16(lane_base + T_ACC + KP + cb, bq);
             tmem_wait_ld();
-            float* sa = slab + (size_t)t * KP + 16 * cg;
+            float* sa = slab + (size_t)t * KP + cb;
             float* sb = sa + (size_t)128 * KP;
 #pragma unroll
             for (int j = 0; j < 16; j += 4) {
@@ -666,37 +738,50 @@ k_w_update_split(const float* __restrict__ slab, float* __restrict__ W, int N, i
 // host side
 // --------------------------------------------------------------------------------------------------------------------
 inline int kp_of(int K) { return (K + 15) / 16 * 16; }
-inline int npt_h(int KP) { return (2 * KP + 3 * KP / 2 + 128 <= 512) ? 3 : 2; }
-inline int npt_w(int KP) { return (3 * KP / 2 + 128 <= 256) ? 3 : 2; }
-inline size_t smem_fixed_h(int NF, int KP) {
-    return (size_t)3 * KP * NF * 2 + (npt_h(KP) == 2 ? (size_t)(KP / 8) * HS_SB : 0) + B_COUNT * 8 + 16;
+// groups of element-wise warps: four chunks in flight where at least two pieces of the TMEM-resident operand still fit
+inline int ng_of(int KP) { return KP <= 80 ? 4 : 2; }
+inline size_t smem_fixed_h(int NF, int KP, int NG) {
+    return (size_t)3 * KP * NF * 2 + (size_t)(3 - npt_of(KP, NG, 2 * KP)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
 }
-inline size_t smem_fixed_w(int KP) {
-    return (size_t)(3 + (npt_w(KP) == 2 ? 1 : 0)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
+inline size_t smem_fixed_w(int KP, int NG, int HB) {
+    return (size_t)(3 * HB + 3 - npt_of(KP, NG, 2 * KP)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
 }
 inline int slots_for(size_t fixed, int slot_bytes) {
     long long ns = ((long long)SMEM_MAX - (long long)fixed) / slot_bytes;
     return (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
 }
+// the H tile pieces are double-buffered in k_tc_w when at least three ring slots remain
+inline int hb_of(int KP, int NG) { return slots_for(smem_fixed_w(KP, NG, 2), SLOTW) >= 3 ? 2 : 1; }
 
-template <int KS>
-cudaError_t launch_h(const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(k_tc_h<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+// the opt-in shared-memory size is a per-device function attribute: set once per device and instantiation
+template <typename Kern>
+cudaError_t set_smem_attr_once(Kern kern, bool (&done)[NMF_MAX_DEVICES], int device) {
+    if (device >= 0 && device < NMF_MAX_DEVICES && done[device]) return cudaSuccess;
+    cudaError_t e = cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+    if (e == cudaSuccess && device >= 0 && device < NMF_MAX_DEVICES) done[device] = true;
+    return e;
+}
+template <int KS, int NG>
+cudaError_t launch_h(const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
+    static bool done[NMF_MAX_DEVICES] = {};
+    cudaError_t e = set_smem_attr_once(k_tc_h<KS, NG>, done, device);
     if (e != cudaSuccess) return e;
-    k_tc_h<KS><<<grid, THREADS, smem, st>>>(a);
+    k_tc_h<KS, NG><<<grid, 32 * (4 * NG + 2), smem, st>>>(a);
     return cudaSuccess;
 }
-template <int KS>
-cudaError_t launch_w(const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st) {
-    cudaError_t e = cudaFuncSetAttribute(k_tc_w<KS>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)SMEM_MAX);
+template <int KS, int NG>
+cudaError_t launch_w(const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
+    static bool done[NMF_MAX_DEVICES] = {};
+    cudaError_t e = set_smem_attr_once(k_tc_w<KS, NG>, done, device);
     if (e != cudaSuccess) return e;
-    k_tc_w<KS><<<grid, THREADS, smem, st>>>(a);
+    k_tc_w<KS, NG><<<grid, 32 * (4 * NG + 2), smem, st>>>(a);
     return cudaSuccess;
 }
+// KS = 1 .. 5 (KP <= 80) run with four groups, KS = 6 .. 8 with two (ng_of)
 #define NMF_KS_SWITCH(fn, KS, ...)                                    \
-    ((KS) == 1 ? fn<1>(__VA_ARGS__) : (KS) == 2 ? fn<2>(__VA_ARGS__) : (KS) == 3 ? fn<3>(__VA_ARGS__) : \
-     (KS) == 4 ? fn<4>(__VA_ARGS__) : (KS) == 5 ? fn<5>(__VA_ARGS__) : (KS) == 6 ? fn<6>(__VA_ARGS__) : \
-     (KS) == 7 ? fn<7>(__VA_ARGS__) : fn<8>(__VA_ARGS__))
+    ((KS) == 1 ? fn<1, 4>(__VA_ARGS__) : (KS) == 2 ? fn<2, 4>(__VA_ARGS__) : (KS) == 3 ? fn<3, 4>(__VA_ARGS__) : \
+     (KS) == 4 ? fn<4, 4>(__VA_ARGS__) : (KS) == 5 ? fn<5, 4>(__VA_ARGS__) : (KS) == 6 ? fn<6, 2>(__VA_ARGS__) : \
+     (KS) == 7 ? fn<7, 2>(__VA_ARGS__) : fn<8, 2>(__VA_ARGS__))
 
 // persistent CTAs for `n_tiles` tiles on `avail` SMs, evened out so that every CTA gets `per` or `per - 1` tiles
 inline int even_ctas(long long n_tiles, long long avail) {
@@ -708,18 +793,19 @@ inline int even_ctas(long long n_tiles, long long avail) {
 
 // iters x { W half-step (+ optionally the H half-step before it) ; reduce + update }
 int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int rows, int iters, int batch, bool fit) {
-    const int KP = kp_of(p->K), KS = KP / 16;
+    const int KP = kp_of(p->K), KS = KP / 16, NG = ng_of(KP);
     const int MT = (rows + 127) / 128;
     const long long n_tiles = (p->P + TILE - 1) / TILE;
     const long long trows = (long long)batch * rows;
     SplitArgs h{}, w{};
     h.W = w.W = W; h.H = w.H = H; w.slab = h.slab = reinterpret_cast<float*>(p->ws);
     h.N = w.N = rows; h.K = w.K = p->K; h.P = w.P = p->P; h.n_tiles = w.n_tiles = n_tiles;
-    h.NF = w.NF = (rows + FCH - 1) / FCH * FCH; h.NC = w.NC = h.NF / FCH; h.KH = (p->K + 31) / 32; w.KH = (p->K + 63) / 64;
-    h.NS = slots_for(smem_fixed_h(h.NF, KP), SLOT); w.NS = slots_for(smem_fixed_w(KP), SLOTW);
-    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 64, TILE, 0) &&
+    h.NF = w.NF = (rows + FCH - 1) / FCH * FCH; h.NC = w.NC = h.NF / FCH;
+    h.HB = w.HB = hb_of(KP, NG);
+    h.NS = slots_for(smem_fixed_h(h.NF, KP, NG), SLOT); w.NS = slots_for(smem_fixed_w(KP, NG, w.HB), SLOTW);
+    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 32, TILE, 0) &&
               make_map(&w.mX, X, trows, p->P, 128, PSW, 128) && make_map(&w.mO, Om, trows, p->P, 128, PSW, 128);
-    if (fit) ok = ok && make_map(&h.mH, H, (long long)batch * p->K, p->P, 32, TILE, 0) &&
+    if (fit) ok = ok && make_map(&h.mH, H, (long long)batch * p->K, p->P, 16, TILE, 0) &&
                   make_map(&h.mX, X, trows, p->P, FCH, TILE, 0) && make_map(&h.mO, Om, trows, p->P, FCH, TILE, 0);
     if (!ok) {
         if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
@@ -727,17 +813,20 @@ int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, 
     }
     const int ctas_h = even_ctas(n_tiles, p->num_sms / batch);
     const int ctas_w = even_ctas(n_tiles, p->num_sms / (batch * MT));
-    const size_t smem_h = smem_fixed_h(h.NF, KP) + (size_t)h.NS * SLOT, smem_w = smem_fixed_w(KP) + (size_t)w.NS * SLOTW;
+    const size_t smem_h = smem_fixed_h(h.NF, KP, NG) + (size_t)h.NS * SLOT;
+    const size_t smem_w = smem_fixed_w(KP, NG, w.HB) + (size_t)w.NS * SLOTW;
     const int nk = rows * p->K;
-    for (int it = 0; it < iters; ++it) {
+    int rc = nmf_run_iterations(p, fit ? 40 : 41, X, Om, W, H, nullptr, rows, batch, iters, [&]() -> int {
         if (fit) {
-            NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_h, KS, h, dim3(ctas_h, batch), smem_h, p->stream));
+            NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_h, KS, h, dim3(ctas_h, batch), smem_h, p->stream, p->device));
             p->launches++;
         }
-        NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_w, KS, w, dim3(ctas_w, batch, MT), smem_w, p->stream));
+        NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_w, KS, w, dim3(ctas_w, batch, MT), smem_w, p->stream, p->device));
         k_w_update_split<<<dim3((nk + WU_E - 1) / WU_E, batch), WU_E * WU_Q, 0, p->stream>>>(w.slab, W, rows, p->K, KP, ctas_w, MT);
         p->launches += 2;
-    }
+        return NMF_OK;
+    });
+    if (rc) return rc;
     NMF_CUDA_TRY(p, cudaGetLastError());
     return NMF_OK;
 }
@@ -748,8 +837,8 @@ void nmf_tcsplit_configure(nmf_plan* p) {
     p->s_ok = false;
     if (p->K > 128 || p->N > 256) return;
     if (p->P + TILE >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
-    const int KP = kp_of(p->K), NF = (p->N + FCH - 1) / FCH * FCH;
-    if (slots_for(smem_fixed_h(NF, KP), SLOT) < 2 || slots_for(smem_fixed_w(KP), SLOTW) < 2) return;
+    const int KP = kp_of(p->K), NG = ng_of(KP), NF = (p->N + FCH - 1) / FCH * FCH;
+    if (slots_for(smem_fixed_h(NF, KP, NG), SLOT) < 2 || slots_for(smem_fixed_w(KP, NG, hb_of(KP, NG)), SLOTW) < 2) return;
     p->s_ok = true;
 }
 
