@@ -378,6 +378,64 @@ def run_configs(args):
     print(json.dumps({"configs": out}))
 
 
+def run_trace(args):
+    """--trace: timeline of one persistent CTA of the split tensor-core kernels at the metric's shape.  Builds the
+    library with -DNMF_TC_TRACE (paper_2309_04623_b200/build/libnmf_trace.so; the product library is untouched), runs
+    one fit iteration (k_tc_h, k_tc_w) on random data of the workload's shape and prints, as markdown, where the
+    element-wise groups and the MMA issuer of CTA (0, 0, 0) spent their cycles (steady-state tiles only)."""
+    import ctypes
+    import torch
+    from paper_2309_04623_b200 import build as nmf_build, nmf
+    nmf.LIB_PATH = nmf_build.build_trace()
+    torch.cuda.set_device(0)
+    wl = WORKLOADS[args.workload]
+    N, P, K = wl["N"], wl["S"] * wl["S"], wl["K"]
+    plan = nmf.Plan(N, P, K, variant=4)
+    X = torch.rand(N, P, device="cuda") * 10
+    Om = torch.rand(N, P, device="cuda"); Om = Om * (Om > 0.1)
+    W = torch.rand(N, K, device="cuda") + 0.1
+    H = torch.rand(K, P, device="cuda") + 0.1
+    L = nmf.lib()
+    NW, LEN = 18, 2048
+    counts = (ctypes.c_uint * (2 * NW))()
+    events = (ctypes.c_ulonglong * (2 * NW * LEN))()
+    L.nmf_debug_trace.argtypes = [ctypes.c_void_p, ctypes.c_void_p, ctypes.c_int]
+    plan.fit(X, Om, W, H, 2); torch.cuda.synchronize()
+    L.nmf_debug_trace(counts, events, 1)
+    plan.fit(X, Om, W, H, 1); torch.cuda.synchronize()
+    L.nmf_debug_trace(counts, events, 1)
+    names = {1: "slot landed", 2: "S ready", 3: "S loaded", 4: "piece columns free", 5: "chunk handed over",
+             6: "H pieces begin", 7: "H pieces done", 8: "update begin", 9: "update done",
+             16: "chunk ready", 17: "chunk MMAs issued", 18: "S series issued", 19: "H pieces ready"}
+    print(f"# Timeline of CTA (0,0,0), split tensor-core kernels, N={N} P={P} K={K} (cycles of clock64)\n")
+    print("Command: `python bench.py --trace` (builds build/libnmf_trace.so with -DNMF_TC_TRACE; one fit iteration on random data)\n")
+    for ki, kern in enumerate(("k_tc_h", "k_tc_w")):
+        print(f"## {kern}\n")
+        per_warp = {}
+        for w in range(NW):
+            ev = [events[(ki * NW + w) * LEN + i] for i in range(min(counts[ki * NW + w], LEN))]
+            ev = [((e >> 56) & 0xff, (e >> 48) & 0xff, e & 0xffffffffffff) for e in ev]
+            if ev:
+                per_warp[w] = ev
+        if not per_warp:
+            print("(no events)\n"); continue
+        t_all = [t for ev in per_warp.values() for _, _, t in ev]
+        span = max(t_all) - min(t_all)
+        print(f"events recorded over {span} cycles (log capacity {LEN} events per warp)\n")
+        print("| warp | role | mean cycles between consecutive events (from -> to: mean x count) |")
+        print("|---|---|---|")
+        for w, ev in sorted(per_warp.items()):
+            gaps = {}
+            for (e0, a0, t0), (e1, a1, t1) in zip(ev[len(ev) // 4:], ev[len(ev) // 4 + 1:]):     # skip the start-up quarter
+                gaps.setdefault((e0, e1), []).append(t1 - t0)
+            role = "MMA issuer" if any(e >= 16 for e, _, _ in ev) else f"element-wise, group {w // 4}, quadrant {w % 4}"
+            txt = "; ".join(f"{names.get(a, a)} -> {names.get(b, b)}: {sum(v) / len(v):.0f} x {len(v)}"
+                            for (a, b), v in sorted(gaps.items(), key=lambda kv: -sum(kv[1]))[:8])
+            if w % 4 == 0 or role == "MMA issuer":
+                print(f"| {w} | {role} | {txt} |")
+        print()
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
@@ -390,12 +448,16 @@ def main():
     ap.add_argument("--cpu-budget", type=float, default=420.0,
                     help="--impl reference: seconds of oracle steps allowed at full size before falling back to a crop")
     ap.add_argument("--configs", action="store_true", help="print the fit-iteration rate of every config and exit")
+    ap.add_argument("--trace", action="store_true", help="print the tile timeline of the split tensor-core kernels (markdown) and exit")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
-    if args.configs:
+    if args.trace:
+        if rank == 0:
+            run_trace(args)
+    elif args.configs:
         if rank == 0:
             run_configs(args)
     elif args.impl == "reference":

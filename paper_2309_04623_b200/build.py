@@ -57,8 +57,8 @@ def build(force: bool = False, verbose: bool = False) -> str:
 
 
 def build_trace() -> str:
-    """libnmf_trace.so: the same library with the tile-timeline instrumentation of nmf_tcfit.cu compiled in
-    (-DNMF_TC_TRACE; exports nmf_debug_tc_trace).  Used by `python bench.py --trace` only."""
+    """build/libnmf_trace.so: the same library with the timeline instrumentation of the split tensor-core kernels
+    compiled in (-DNMF_TC_TRACE; exports nmf_debug_trace).  Used by `python bench.py --trace` only."""
     os.makedirs(OBJ, exist_ok=True)
     lib = os.path.join(OBJ, "libnmf_trace.so")
     with cf.ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
@@ -69,5 +69,24 @@ def build_trace() -> str:
     return lib
 
 
+def build_wait_debug() -> str:
+    """build/libnmf_waitdebug.so: the same library with -DNMF_WAIT_DEBUG: an mbarrier wait that times out is logged
+    (nmf_debug_wait_log) and abandoned instead of trapping.  A debugging aid for protocol errors; not used by the
+    product, the tests or bench.py."""
+    os.makedirs(OBJ, exist_ok=True)
+    lib = os.path.join(OBJ, "libnmf_waitdebug.so")
+    with cf.ThreadPoolExecutor(max_workers=min(8, len(SOURCES))) as ex:
+        objs = list(ex.map(lambda s: _compile(s, False, False, ("-DNMF_WAIT_DEBUG",), ".waitdebug"), SOURCES))
+    if not os.path.exists(lib) or os.path.getmtime(lib) < max(os.path.getmtime(o) for o in objs):
+        subprocess.check_call(["nvcc", "-shared", "-gencode", "arch=compute_100a,code=sm_100a",
+                               "-o", lib, *objs, "-cudart", "static", "-lcuda"])
+    return lib
+
+
 if __name__ == "__main__":
-    print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))
+    if "--wait-debug" in sys.argv:
+        print(build_wait_debug())
+    elif "--trace" in sys.argv:
+        print(build_trace())
+    else:
+        print(build(force="--force" in sys.argv, verbose="-v" in sys.argv))

@@ -51,15 +51,70 @@ __device__ __forceinline__ bool mbar_try_wait_hint(uint64_t* bar, uint32_t parit
 // suspend-time-hint form compiles to TRYWAIT + NANOSLEEP.SYNCS + a second probe and woke about twenty times per
 // wait: a third of all instructions the element-wise warps issued); 2^26 failed probes are far beyond any legitimate
 // wait (a whole launch takes milliseconds).
+#ifdef NMF_WAIT_DEBUG
+// debugging build (python -m paper_2309_04623_b200.build --wait-debug): a wait that times out is recorded (block, warp,
+// shared-memory address of the barrier, parity) and abandoned instead of trapping, so the log survives the launch
+__device__ unsigned int g_wait_log[4 * 256];
+__device__ unsigned int g_wait_log_n;
+#endif
 __device__ __forceinline__ void mbar_wait(uint64_t* bar, uint32_t parity) {
     uint32_t n = 0;
     while (!mbar_try_wait(bar, parity)) {
+#ifdef NMF_WAIT_DEBUG
+        if (++n > (1u << 22)) {
+            if ((threadIdx.x & 31) == 0 || true) {
+                const unsigned int i = atomicAdd(&g_wait_log_n, 1u);
+                if (i < 256) {
+                    g_wait_log[4 * i] = blockIdx.x | (blockIdx.y << 12) | (blockIdx.z << 24);
+                    g_wait_log[4 * i + 1] = threadIdx.x;
+                    g_wait_log[4 * i + 2] = smem_u32(bar);
+                    g_wait_log[4 * i + 3] = parity;
+                }
+            }
+            return;
+        }
+#else
         if (++n > (1u << 26)) __trap();
+#endif
     }
 }
 __device__ __forceinline__ void mbar_expect_tx(uint64_t* bar, uint32_t bytes) {
     asm volatile("mbarrier.arrive.expect_tx.shared::cta.b64 _, [%0], %1;" ::"r"(smem_u32(bar)), "r"(bytes) : "memory");
 }
+
+// ---------------------------------------------------------------- timeline trace (python bench.py --trace)
+// With -DNMF_TC_TRACE (build.py build_trace) lane 0 of every warp of CTA (0, 0, 0) records (event, argument, clock64)
+// at the hand-over points of the split kernels; nmf_debug_trace copies the log out.  Compiled out of the product.
+#ifdef NMF_TC_TRACE
+constexpr int TRACE_WARPS = 18, TRACE_LEN = 2048, TRACE_KERNELS = 2;
+__device__ unsigned long long g_trace[TRACE_KERNELS * TRACE_WARPS * TRACE_LEN];
+__device__ unsigned int g_trace_n[TRACE_KERNELS * TRACE_WARPS];
+// the event counter lives in a register of the recording lane (a counter in global memory cost a round trip per event)
+__device__ __forceinline__ void trace_event(int kern, int warp, int lane, unsigned& n, unsigned ev, unsigned arg) {
+    if (lane == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0 && n < TRACE_LEN) {
+        g_trace[(kern * TRACE_WARPS + warp) * TRACE_LEN + n] =
+            ((unsigned long long)ev << 56) | ((unsigned long long)(arg & 0xffu) << 48) | ((unsigned long long)clock64() & 0xffffffffffffULL);
+        ++n;
+    }
+}
+__device__ __forceinline__ void trace_flush(int kern, int warp, int lane, unsigned n) {
+    if (lane == 0 && blockIdx.x == 0 && blockIdx.y == 0 && blockIdx.z == 0) g_trace_n[kern * TRACE_WARPS + warp] = n;
+}
+#define NMF_TRC_DECL unsigned trc_n = 0
+#define NMF_TRC(ev, arg) tc::trace_event(0, warp, lane, trc_n, (ev), (arg))
+#define NMF_TRCW(ev, arg) tc::trace_event(1, warp, lane, trc_n, (ev), (arg))
+#define NMF_TRC_FLUSH(kern) tc::trace_flush((kern), warp, lane, trc_n)
+#else
+#define NMF_TRC_DECL do { } while (0)
+#define NMF_TRC(ev, arg) do { } while (0)
+#define NMF_TRCW(ev, arg) do { } while (0)
+#define NMF_TRC_FLUSH(kern) do { } while (0)
+#endif
+// trace events: element-wise warps 1 slot landed, 2 S ready, 3 S loaded, 4 piece columns free, 5 pieces stored + chunk
+// handed over, 6 H pieces begin, 7 H pieces done, 8 update begin, 9 update done; MMA issuer 16 pieces of a chunk ready,
+// 17 its MMAs issued, 18 S series issued, 19 H pieces ready
+enum { TR_FULL = 1, TR_S, TR_LD, TR_EFREE, TR_HANDED, TR_H0_BEGIN, TR_H0_END, TR_UPD_BEGIN, TR_UPD_END,
+       TR_M_READY = 16, TR_M_ISSUED, TR_M_S, TR_M_HS };
 
 // ---------------------------------------------------------------- TMA (cp.async.bulk.tensor, 2-D tiled maps)
 // Loads the box of `tmap` whose first element is (x = innermost coordinate, y = row) into shared memory at
@@ -68,12 +123,6 @@ __device__ __forceinline__ void tma_load_2d(uint32_t smem_dst, const void* tmap,
     asm volatile(
         "cp.async.bulk.tensor.2d.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1, {%2, %3}], [%4];"
         ::"r"(smem_dst), "l"(reinterpret_cast<uint64_t>(tmap)), "r"(x), "r"(y), "r"(smem_u32(bar)) : "memory");
-}
-// The same box is only brought into L2 (no shared-memory destination, no completion to wait for): issued a few tiles
-// ahead of the load, so that the bytes in flight from HBM wait in L2 and not in ring slots.
-__device__ __forceinline__ void tma_prefetch_l2_2d(const void* tmap, int x, int y) {
-    asm volatile("cp.async.bulk.prefetch.tensor.2d.L2.global.tile [%0, {%1, %2}];"
-                 ::"l"(reinterpret_cast<uint64_t>(tmap)), "r"(x), "r"(y) : "memory");
 }
 __device__ __forceinline__ void tma_prefetch_desc(const void* tmap) {
     asm volatile("prefetch.tensormap [%0];" ::"l"(reinterpret_cast<uint64_t>(tmap)) : "memory");

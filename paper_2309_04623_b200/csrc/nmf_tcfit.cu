@@ -116,7 +116,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         mbar_init(&bars[B_S20], 1); mbar_init(&bars[B_S21], 1); mbar_init(&bars[B_WT], EW_WARPS);
         mbar_init(&bars[B_P20], 4); mbar_init(&bars[B_P21], 4); mbar_init(&bars[B_AB], 1);
         mbar_init(&bars[B_ABG0], 1); mbar_init(&bars[B_ABG1], 1);
-        for (uint32_t s = 0; s < NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 4); }
+        for (uint32_t s = 0; s < NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], EW_WARPS); }
         mbar_fence_init();
     }
     if (warp == W_MMA) tmem_alloc(tptr, 512);
@@ -321,6 +321,11 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[bar]);
         };
+        // An mbarrier wait tests a phase PARITY, so a warp may only test the "full" barrier of a slot for use u if it
+        // also saw use u - 1 (a group that ran ahead of a late TMA load would see the parity of use u - 2 and read a
+        // slot that has not landed).  Every element-wise warp therefore waits for and releases EVERY slot, in ring
+        // order: the slots of the other group are only observed.
+        auto observe = [&](uint32_t seq) { wait_full(seq); release(seq); };
         // rows 128 m .. 128 m + 127 of the W pieces -> TMEM (A operand of S'): group 0 stages pieces 0 and 1, group 1 piece 2
         auto stage_wt = [&](int m) {
             const int fr = 128 * m + t;
@@ -368,6 +373,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 *reinterpret_cast<uint4*>(hs_p + 2 * HS_BYTES + off) = make_uint4(hp3[4 * gq], hp3[4 * gq + 1], hp3[4 * gq + 2], hp3[4 * gq + 3]);
             }
             if (grp < KH) release(sq + grp);
+            if (1 - grp < KH) observe(sq + 1 - grp);
             if (proj) { stage_wt(0); tc_fence_before(); }        // (the previous tile's MMAs are complete: B_AB)
             fence_proxy_async();
             warp_arrive(B_HS);
@@ -378,6 +384,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             for (int j = 0; j < NSC; ++j) {
                 const int c = 2 * j + grp;
                 const bool have = c < NC;
+                if (grp == 1) observe(sq + KH + c - 1);  // group 0's chunk of this super-chunk comes first in the ring
                 float x[16], o[16];
                 if (have) {
                     const uint32_t seq = sq + KH + c;
@@ -406,6 +413,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     warp_arrive(B_P0 + grp);
                     pending = true;
                 }
+                if (grp == 0 && c + 1 < NC) observe(sq + KH + c + 1);
             }
             // ---- UPD: h' = h * num / max(den, eps); thread = (pixel t, this group's 32 comps) ----
             // the old h is rebuilt exactly from its three BF16 pieces in Hs (h = h1 + h2 + h3, every partial sum exact)
@@ -465,6 +473,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 for (int j = 0; j < NSC2; ++j) {
                     const int c = 2 * j + grp;
                     const uint32_t seq = sq + KH + NCR + NCH2 * m + c;
+                    if (grp == 1) observe(seq - 1);
                     const unsigned char* xsl = wait_full(seq);       // X rows at +0, Omega rows at +8 KB
                     float x[16], o[16];
                     if (active) {
@@ -498,6 +507,7 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                     tc_fence_before();
                     warp_arrive(B_P20 + grp);
                     pending = true;
+                    if (grp == 0) observe(seq + 1);
                 }
             }
             wait(B_ABG0 + grp);

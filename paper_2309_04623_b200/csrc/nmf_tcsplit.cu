@@ -15,10 +15,17 @@
 //               written as soon as the last S of a tile has completed, before the H update of that tile.
 //   k_tc_w<KS,NG>  W half-step (a6-a7) with the new H.  TMEM lane = frame.  One 128-frame M tile per CTA
 //               (blockIdx.z), so a CTA keeps 2 KP accumulator columns and its M tile's rows of W stay in TMEM for
-//               the whole launch.  The H tile pieces are double-buffered in shared memory when they fit.  X and
-//               Omega rows are read only by the CTAs of their M tile.  Also the projection kernel (a9) with
+//               the whole launch.  X and Omega rows are read only by the CTAs of their M tile; the ring is as deep
+//               as shared memory allows (the kernel waited for data, not for the tensor pipe).  Also the projection kernel (a9) with
 //               X = targets, Omega = omega, W = coef.
 //   k_w_update_split   fixed-order fp64 reduction of the per-CTA slabs + W <- W o A / max(B, eps)  (a8)
+//
+// Ring slots and groups.  An mbarrier wait tests a phase PARITY, so a consumer may only test the "full" barrier of a
+// slot for use u if it also consumed use u - 1 (a group that ran ahead of a late TMA load saw the parity of use
+// u - 2 and read a slot that had not landed: tx-count corruption, launch failure at N = 200, K = 100, where the ring had
+// three slots).  In k_tc_h work items are therefore dealt to the groups by their ring sequence number (item seq -> group
+// seq % NG) and the number of slots is a multiple of NG: every use of a slot then belongs to the same group.  In k_tc_w
+// (few, large slots) every element-wise warp waits for and releases every slot, in ring order, and reads only its own.
 //
 // X and Omega cross HBM twice per iteration instead of once (the fused kernel re-reads them through L2).
 // Arithmetic and operand layouts are those of nmf_tcfit.cu (BF16x3 split, six piece products per product, FP32
@@ -36,13 +43,13 @@ constexpr int PCH = 16;                   // pixels per W-step chunk
 constexpr int HS_SB = 16 * 128;           // [128 rows][comps] piece buffers: bytes between 8-component groups
 constexpr int SLOT = 16384;               // k_tc_h ring slot: [16 frames][128 px] of X and of Omega, or [16 comps][128 px] of H
 constexpr int PSW = 32;                   // k_tc_w: pixels per X / Omega ring slot (two W-step chunks)
-constexpr int SLOTW = 32768;              // k_tc_w ring slot: [128 frames][32 px] of X and of Omega, or [32 comps][128 px] of H
-constexpr int MAX_SLOTS = 10;
+constexpr int SLOTW = 32768;              // k_tc_w ring slot: [128 frames][32 px] of X and of Omega, or [64 comps][128 px] of H
+constexpr int MAX_SLOTS = 12;
 constexpr int MAX_NG = 4;
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 struct SplitArgs {
-    CUtensorMap mH;            // H   [B*K, P]  box [16 comps][128 px] (k_tc_h) or [32 comps][128 px] (k_tc_w)
+    CUtensorMap mH;            // H   [B*K, P]  box [16 comps][128 px] (k_tc_h) or [64 comps][128 px] (k_tc_w)
     CUtensorMap mX, mO;        // X, Om [B*rows, P]: box [16 frames][128 px] (k_tc_h) or [128 frames][32 px], 128-byte swizzle
                                // (k_tc_w: full 128-byte lines from HBM; 64-byte rows ran the kernel at a quarter of the HBM rate)
     const float* W; float* H; float* slab;
@@ -50,7 +57,6 @@ struct SplitArgs {
     int NF;                    // frames padded to a multiple of 16
     int NC;                    // H-step chunks = NF / 16
     int NS;                    // ring slots
-    int HB;                    // k_tc_w: buffers of the H tile pieces in shared memory (1 or 2)
 };
 
 enum { B_HS = 0, B_UPD, B_S0, B_S1, B_DONE, B_P0, B_G0 = B_P0 + MAX_NG, B_FULL = B_G0 + MAX_NG,
@@ -125,6 +131,7 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const int b = blockIdx.y;
+    NMF_TRC_DECL;
     const float* __restrict__ W = g.W + (size_t)b * N * K;
     float* __restrict__ H = g.H + (size_t)b * K * P;
 
@@ -173,19 +180,11 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
                 ++seq;
                 return s;
             };
-            // L2 prefetch of a whole tile's boxes (H blocks, X and Omega chunks), one tile ahead of the ring loads
-            auto prefetch_tile = [&](long long tile) {
-                if (tile >= g.n_tiles) return;
-                const int p0 = (int)(tile * TILE);
-                for (int h = 0; h < NBLK; ++h) tma_prefetch_l2_2d(&g.mH, p0, b * K + 16 * h);
-                for (int c = 0; c < NC; ++c) {
-                    tma_prefetch_l2_2d(&g.mX, p0, b * N + FCH * c);
-                    tma_prefetch_l2_2d(&g.mO, p0, b * N + FCH * c);
-                }
-            };
+            // (bringing the data of the tiles ahead into L2 -- cp.async.bulk.prefetch.tensor a tile at a time or item by
+            // item, or plain prefetch.global.L2 instructions from an extra warp -- made both kernels 20 - 50 % slower
+            // on the box and was dropped)
             for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
                 const int p0 = (int)(tile * TILE);
-                prefetch_tile(tile + gridDim.x);
                 for (int h = 0; h < NBLK; ++h) {
                     const uint32_t s = acquire(16 * TILE * 4);
                     tma_load_2d(ring_s + s * SLOT, &g.mH, p0, b * K + 16 * h, &bars[B_FULL + s]);
@@ -212,7 +211,9 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
         const uint32_t ws_kstep = (uint32_t)(2 * WS_SB) >> 4;
         constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
         bool first = true;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+        uint32_t sq = 0;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
+            const int og = (int)((sq + NBLK) & (NG - 1));        // chunk c of this tile belongs to group (og + c) % NG
             auto issue_S = [&](int j) {                  // S(j): [128 px] x [16 NG frames], K = comps -> Z[j & 1]
                 if (elect_one()) {
                     const uint32_t d = tmem + T_Z + 16 * NG * (j & 1);
@@ -232,17 +233,21 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
                 __syncwarp();
             };
             wait(B_HS);
+            NMF_TRC(TR_M_HS, 0);
             issue_S(0);
             if (NSC > 1) issue_S(1);
+            NMF_TRC(TR_M_S, 1);
             if (!first) wait(B_UPD);                     // the previous tile's update has read Num / Den
             first = false;
             for (int j = 0; j < NSC; ++j) {
-                for (int gg = 0; gg < NG; ++gg) {
-                    const int c = NG * j + gg;
+                for (int gi = 0; gi < NG; ++gi) {            // gi: position of the chunk in its super-chunk
+                    const int c = NG * j + gi;
                     if (c >= NC) break;
+                    const int gg = (og + gi) & (NG - 1);     // the group that prepares this chunk
                     wait(B_P0 + gg);
+                    NMF_TRC(TR_M_READY, c);
                     if (elect_one()) {
-                        const uint32_t z = tmem + T_Z + 16 * NG * (j & 1) + 16 * gg, e = tmem + T_E + 32 * gg;
+                        const uint32_t z = tmem + T_Z + 16 * NG * (j & 1) + 16 * gi, e = tmem + T_E + 32 * gg;
                         const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
                         const uint32_t a_r[3] = {z, z + 8, e + O_R3};
                         const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 frames = 2 row groups
@@ -255,8 +260,9 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
                         mma_commit(&bars[B_G0 + gg]);
                     }
                     __syncwarp();
+                    NMF_TRC(TR_M_ISSUED, c);
                 }
-                if (j + 2 < NSC) issue_S(j + 2);
+                if (j + 2 < NSC) { issue_S(j + 2); NMF_TRC(TR_M_S, j + 2); }
             }
             if (elect_one()) mma_commit(&bars[B_DONE]);
             __syncwarp();
@@ -283,12 +289,14 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[bar]);
         };
-        // H0: the pieces of a tile's H -> TMEM / shared memory (A operand of S); group g takes the 16-component blocks
-        // g, g + NG, ... (one ring slot each) and keeps their fp32 values for the update
+        // H0: the pieces of a tile's H -> TMEM / shared memory (A operand of S); a group takes the 16-component blocks
+        // (one ring slot each) whose ring sequence number sqt + bi is its own modulo NG, and keeps their fp32 values
+        // for the update
         auto h0 = [&](uint32_t sqt, float (&hv)[NB][16]) {
+            NMF_TRC(TR_H0_BEGIN, 0);
 #pragma unroll
             for (int bb = 0; bb < NB; ++bb) {
-                const int bi = grp + NG * bb;
+                const int bi = (int)((grp - sqt) & (NG - 1)) + NG * bb;
                 if (bi < NBLK) {
                     const float* hsl = reinterpret_cast<const float*>(wait_full(sqt + bi)) + t;
                     uint32_t p[3][8];
@@ -308,28 +316,35 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             if (NPT < 3) fence_proxy_async();
             tc_fence_before();
             warp_arrive(B_HS);
+            NMF_TRC(TR_H0_END, 0);
         };
         float hold[NB][16];
         uint32_t sq = 0;
         h0(0, hold);
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
-            // ---- steps: super-chunk j = chunks NG j + grp; thread = (pixel t, 16 frames), two halves of 8 ----
+            // ---- steps: this group's chunk of super-chunk j is NG j + zp (its ring slot has the group's sequence
+            // number modulo NG); thread = (pixel t, 16 frames), two halves of 8 ----
             bool pending = false;
+            const int zp = (int)((grp - (sq + NBLK)) & (NG - 1));
             for (int j = 0; j < NSC; ++j) {
-                const int c = NG * j + grp;
+                const int c = NG * j + zp;
                 const bool have = c < NC;
                 const float* xs = nullptr;
                 if (have) xs = reinterpret_cast<const float*>(wait_full(sq + NBLK + c)) + t;
+                NMF_TRC(TR_FULL, c);
                 wait(B_S0 + (j & 1));                    // every group tracks every completion of the buffer's barrier
+                NMF_TRC(TR_S, c);
                 if (have) {
                     tc_fence_after();
-                    const uint32_t zcol = lane_base + T_Z + 16 * NG * (j & 1) + 16 * grp;
+                    const uint32_t zcol = lane_base + T_Z + 16 * NG * (j & 1) + 16 * zp;
                     const uint32_t ecol = lane_base + T_E + 32 * grp;
                     const int nv = N - FCH * c;          // valid frames of this chunk (>= 16: all)
                     uint32_t s[16];
                     tmem_ld16(zcol, s);
                     tmem_wait_ld();
+                    NMF_TRC(TR_LD, c);
                     if (pending) { wait(B_G0 + grp); tc_fence_after(); }      // this group's E columns are free again
+                    NMF_TRC(TR_EFREE, c);
 #pragma unroll
                     for (int hf = 0; hf < 2; ++hf) {
                         float x[8], o[8];
@@ -350,6 +365,7 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
                     tmem_wait_st();
                     tc_fence_before();
                     warp_arrive(B_P0 + grp);
+                    NMF_TRC(TR_HANDED, c);
                     pending = true;
                 }
             }
@@ -363,11 +379,12 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             if (pending) wait(B_G0 + grp);
             wait(B_DONE);                                // Num, Den complete
             tc_fence_after();
+            NMF_TRC(TR_UPD_BEGIN, 0);
             const long long p = tile * TILE + t;
             const bool p_ok = p < P;
 #pragma unroll
             for (int bb = 0; bb < NB; ++bb) {
-                const int kb = 16 * (grp + NG * bb);
+                const int kb = 16 * ((int)((grp - sq) & (NG - 1)) + NG * bb);    // the blocks this thread split in H0
                 if (kb < KP) {                           // (warp-uniform: tcgen05.ld is warp-collective)
                     uint32_t nm[16], dn[16];
                     tmem_ld16(lane_base + T_NUM + kb, nm);
@@ -384,6 +401,7 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             }
             tc_fence_before();
             warp_arrive(B_UPD);
+            NMF_TRC(TR_UPD_END, 0);
             if (has_next) {
                 if constexpr (EARLY) {
 #pragma unroll
@@ -392,6 +410,7 @@ k_tc_h(const __grid_constant__ SplitArgs g) {
             }
         }
     }
+    NMF_TRC_FLUSH(0);
     tc_fence_before();
     __syncthreads();
     if (warp == W_MMA) tmem_dealloc(tmem, 512);
@@ -411,15 +430,15 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     constexpr uint32_t T_ACC = 512 - 2 * KP;                              // A at T_ACC, B at T_ACC + KP
     static_assert(T_E + 32 * NG <= T_ACC, "TMEM");
     constexpr int NBLK = KP / 16;                        // 16-component blocks
-    constexpr int NHS = (NBLK + 1) / 2;                  // H ring slots (32 components each) per tile
+    constexpr int NHS = (NBLK + 3) / 4;                  // H ring slots (64 components each) per tile
     constexpr int NSW = TILE / PSW;                      // X / Omega ring slots per tile
     constexpr int NSC2 = TILE / (PCH * NG);              // super-chunks of 16 NG pixels per tile
     constexpr int HS_BYTES = (KP / 8) * HS_SB;           // one BF16 piece of the H tile / of the M tile's W rows
     extern __shared__ __align__(1024) unsigned char smem[];
-    const int N = g.N, K = g.K, HB = g.HB;
+    const int N = g.N, K = g.K;
     unsigned char* ring = smem;
-    unsigned char* hs_p = ring + (size_t)g.NS * SLOTW;  // HB x 3 pieces of the H tile, [pixel][comp]
-    unsigned char* wsx_p = hs_p + (size_t)HB * 3 * HS_BYTES;     // pieces NPT .. 2 of this M tile's rows of W
+    unsigned char* hs_p = ring + (size_t)g.NS * SLOTW;  // 3 pieces of the H tile, [pixel][comp]
+    unsigned char* wsx_p = hs_p + 3 * HS_BYTES;         // pieces NPT .. 2 of this M tile's rows of W
     uint64_t* bars = reinterpret_cast<uint64_t*>(wsx_p + (3 - NPT) * HS_BYTES);
     uint32_t* tptr = reinterpret_cast<uint32_t*>(bars + B_COUNT);
     const RingCtl rc{(uint32_t)g.NS, 0xffffffffu / (uint32_t)g.NS + 1u};
@@ -427,6 +446,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     const int tid = threadIdx.x, lane = tid & 31;
     const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const int b = blockIdx.y, m = blockIdx.z;
+    NMF_TRC_DECL;
     const float* __restrict__ W = g.W + (size_t)b * N * K;
     // slab of this CTA: [B][MT][ctas][2][128][KP]
     float* slab = g.slab + (((size_t)b * gridDim.z + m) * gridDim.x + blockIdx.x) * 2 * (size_t)128 * KP;
@@ -435,7 +455,8 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
         mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_UPD], 1);     // B_UPD: every MMA of the launch is complete
         mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1); mbar_init(&bars[B_DONE], 1);
         for (int i = 0; i < NG; ++i) { mbar_init(&bars[B_P0 + i], 4); mbar_init(&bars[B_G0 + i], 1); }
-        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], 8); }
+        // every element-wise warp waits for and releases EVERY ring slot (see "Ring slots and groups")
+        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], EW_WARPS); }
         mbar_fence_init();
     }
     if (warp == W_MMA) tmem_alloc(tptr, 512);
@@ -478,6 +499,9 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
     __syncthreads();
     tc_fence_after();
 
+    // Ring order per tile: the H tile (NHS slots of 64 components), then the M tile's rows of X and Omega, 32 pixels
+    // (two chunks) per slot.  The ring is as deep as shared memory allows (five 32 KB slots at K <= 64: one tile ahead):
+    // with four slots, half of them half empty, the element-wise warps waited 3000 cycles per tile for data.
     if (warp == W_TMA) {
         // =========================== TMA producer ===========================
         if (lane == 0) {
@@ -490,24 +514,13 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                 ++seq;
                 return s;
             };
-            // L2 prefetch of a whole tile's boxes, one tile ahead of the ring loads
-            auto prefetch_tile = [&](long long tile) {
-                if (tile >= g.n_tiles) return;
-                const int p0 = (int)(tile * TILE);
-                for (int h = 0; h < NHS; ++h) tma_prefetch_l2_2d(&g.mH, p0, b * K + 32 * h);
-                for (int c = 0; c < NSW; ++c) {
-                    tma_prefetch_l2_2d(&g.mX, p0 + PSW * c, b * N + 128 * m);
-                    tma_prefetch_l2_2d(&g.mO, p0 + PSW * c, b * N + 128 * m);
-                }
-            };
             for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
                 const int p0 = (int)(tile * TILE);
-                prefetch_tile(tile + gridDim.x);
                 for (int h = 0; h < NHS; ++h) {
-                    const uint32_t s = acquire(32 * TILE * 4);
-                    tma_load_2d(ring_s + s * SLOTW, &g.mH, p0, b * K + 32 * h, &bars[B_FULL + s]);
+                    const uint32_t s = acquire(SLOTW);
+                    tma_load_2d(ring_s + s * SLOTW, &g.mH, p0, b * K + 64 * h, &bars[B_FULL + s]);
                 }
-                for (int c = 0; c < NSW; ++c) {          // the M tile's 128 rows of X and Omega, 32 px (two chunks) at a time
+                for (int c = 0; c < NSW; ++c) {
                     const uint32_t s = acquire(SLOTW);
                     tma_load_2d(ring_s + s * SLOTW, &g.mX, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
                     tma_load_2d(ring_s + s * SLOTW + 128 * PSW * 4, &g.mO, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
@@ -527,35 +540,36 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             d_wsx_k[i] = smem_desc(wsx_s + (i >= NPT ? i - NPT : 0) * HS_BYTES, HS_SB, 128);
         }
         constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
+        auto issue_S2 = [&](int j) {                     // S'(j): [128 frames] x [16 NG px], K = comps -> Z[j & 1]
+            if (elect_one()) {
+                const uint32_t boff = (uint32_t)(j * NG * 2 * 128) >> 4;
+                const uint32_t d = tmem + T_Z + 16 * NG * (j & 1);
+#pragma unroll
+                for (int pr = 0; pr < 6; ++pr)
+#pragma unroll
+                    for (int ks = 0; ks < KS; ++ks) {
+                        const uint64_t bd = d_hs_k[PB[pr]] + boff + ks * hs_kstep;
+                        if (PA[pr] < NPT) mma16_ts(d, tmem + T_WT + PA[pr] * (KP / 2) + 8 * ks, bd, id_s, (pr | ks) ? 1u : 0u);
+                        else mma16_ss(d, d_wsx_k[PA[pr]] + ks * hs_kstep, bd, id_s, (pr | ks) ? 1u : 0u);
+                    }
+                mma_commit(&bars[B_S0 + (j & 1)]);
+            }
+            __syncwarp();
+        };
         bool acc_started = false;
-        uint32_t it = 0;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, ++it) {
-            const uint32_t hboff = (HB == 2 && (it & 1u)) ? (uint32_t)(3 * HS_BYTES) >> 4 : 0u;      // this tile's Hs buffer
-            auto issue_S2 = [&](int j) {                 // S'(j): [128 frames] x [16 NG px], K = comps -> Z[j & 1]
-                if (elect_one()) {
-                    const uint32_t boff = hboff + ((uint32_t)(j * NG * 2 * 128) >> 4);
-                    const uint32_t d = tmem + T_Z + 16 * NG * (j & 1);
-#pragma unroll
-                    for (int pr = 0; pr < 6; ++pr)
-#pragma unroll
-                        for (int ks = 0; ks < KS; ++ks) {
-                            const uint64_t bd = d_hs_k[PB[pr]] + boff + ks * hs_kstep;
-                            if (PA[pr] < NPT) mma16_ts(d, tmem + T_WT + PA[pr] * (KP / 2) + 8 * ks, bd, id_s, (pr | ks) ? 1u : 0u);
-                            else mma16_ss(d, d_wsx_k[PA[pr]] + ks * hs_kstep, bd, id_s, (pr | ks) ? 1u : 0u);
-                        }
-                    mma_commit(&bars[B_S0 + (j & 1)]);
-                }
-                __syncwarp();
-            };
-            wait(B_HS);                                  // the new H tile's pieces are in this tile's Hs buffer
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+            wait(B_HS);                                  // the tile's H pieces are in Hs
+            NMF_TRCW(TR_M_HS, 0);
             issue_S2(0);
-            if (NSC2 > 1) issue_S2(1);
+            issue_S2(1);
+            NMF_TRCW(TR_M_S, 1);
             for (int j = 0; j < NSC2; ++j) {
                 for (int gg = 0; gg < NG; ++gg) {
                     const int c = NG * j + gg;
                     wait(B_P0 + gg);
+                    NMF_TRCW(TR_M_READY, c);
                     if (elect_one()) {
-                        const uint32_t boff = hboff + ((uint32_t)(c * 2 * 128) >> 4);   // 16 pixels = 2 row groups
+                        const uint32_t boff = (uint32_t)(c * 2 * 128) >> 4;   // 16 pixels = 2 row groups
                         const uint32_t z = tmem + T_Z + 16 * NG * (j & 1) + 16 * gg, e = tmem + T_E + 32 * gg;
                         const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
                         const uint32_t a_r[3] = {z, z + 8, e + O_R3};
@@ -568,17 +582,14 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                         mma_commit(&bars[B_G0 + gg]);
                     }
                     __syncwarp();
+                    NMF_TRCW(TR_M_ISSUED, c);
                     acc_started = true;
                 }
-                if (j + 2 < NSC2) issue_S2(j + 2);
+                if (j + 2 < NSC2) { issue_S2(j + 2); NMF_TRCW(TR_M_S, j + 2); }
             }
-            if (HB == 1) {                               // single Hs buffer: the next H0 waits for every MMA of this tile
-                if (elect_one()) mma_commit(&bars[B_DONE]);
-                __syncwarp();
-            }
+            if (elect_one()) mma_commit(&bars[B_DONE]);  // every MMA of this tile is complete: Hs may be rewritten
+            __syncwarp();
         }
-        if (elect_one()) mma_commit(&bars[B_UPD]);       // every MMA of the launch is complete
-        __syncwarp();
     } else if (warp < EW_WARPS) {
         // =========================== element-wise warps: group grp = warp / 4, lane quadrant q = warp % 4 ===========================
         const int q = warp & 3, grp = warp >> 2;
@@ -603,47 +614,58 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             __syncwarp();
             if (lane == 0) mbar_arrive(&bars[bar]);
         };
-        // H0: the (new) H tile is split into Hs[buffer][pixel][comp]; thread = pixel t.  Ring slot h holds the
-        // components 32 h .. 32 h + 31: its two 16-component blocks go to the groups (2 h) % NG and (2 h + 1) % NG, so
-        // every slot is released by exactly eight warps, like an X / Omega slot.
-        auto h0 = [&](uint32_t sqt, uint32_t buf) {
-            unsigned char* hb = hs_p + (size_t)buf * 3 * HS_BYTES;
+        // H0: the (new) H tile is split into Hs[pixel][comp]; thread = pixel t; ring slot h holds the components
+        // 64 h .. 64 h + 63, group g takes the block of 16 components g of it (block g % 4 with two groups: two each)
+        auto h0 = [&](uint32_t sqt) {
+            NMF_TRCW(TR_H0_BEGIN, 0);
             for (int h = 0; h < NHS; ++h) {
-                const int sub = (grp - 2 * h) & (NG - 1);            // 0 or 1: this group's block of the slot
-                if (sub < 2) {
-                    const int bi = 2 * h + sub;
-                    const float* hsl = reinterpret_cast<const float*>(wait_full(sqt + h)) + (16 * sub) * TILE + t;
+                const float* hsl = reinterpret_cast<const float*>(wait_full(sqt + h)) + t;
+                for (int sb = grp; sb < 4; sb += NG) {
+                    const int bi = 4 * h + sb;
                     if (bi < NBLK) {
                         uint32_t p[3][8];
-                        split_rows16(hsl, 16 * bi, K, nullptr, p[0], p[1], p[2]);
+                        split_rows16(hsl + (16 * sb) * TILE, 16 * bi, K, nullptr, p[0], p[1], p[2]);
 #pragma unroll
                         for (int i = 0; i < 3; ++i) {
-                            st_piece_smem(hb + i * HS_BYTES, t, 2 * bi, &p[i][0]);
-                            st_piece_smem(hb + i * HS_BYTES, t, 2 * bi + 1, &p[i][4]);
+                            st_piece_smem(hs_p + i * HS_BYTES, t, 2 * bi, &p[i][0]);
+                            st_piece_smem(hs_p + i * HS_BYTES, t, 2 * bi + 1, &p[i][4]);
                         }
                     }
-                    release(sqt + h);
                 }
+                release(sqt + h);
             }
             fence_proxy_async();
             warp_arrive(B_HS);
+            NMF_TRCW(TR_H0_END, 0);
         };
-        uint32_t sq = 0, it = 0;
-        h0(0, 0);
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile, ++it) {
-            // ---- steps: chunk c = NG j + grp of super-chunk j; thread = (frame 128 m + t, 16 pixels), two halves of 8 ----
+        uint32_t sq = 0;
+        bool first = true;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
+            if (!first) wait(B_DONE);                    // every MMA of the previous tile is complete: Hs is free
+            first = false;
+            h0(sq);
+            // ---- steps: chunk c = NG j + grp of super-chunk j lies in ring slot c / 2 (32 pixels); the slots of the other
+            // groups are only observed (waited for and released), in ring order; thread = (frame 128 m + t, 16 pixels),
+            // two halves of 8 ----
             bool pending = false;
             const int sw = t & 7;
+            int sv = 0;                                  // X / Omega slots of this tile visited so far
             for (int j = 0; j < NSC2; ++j) {
                 const int c = NG * j + grp;
-                const uint32_t seq = sq + NHS + (c >> 1);            // ring slot of 32 pixels: chunks 2 s and 2 s + 1
+                for (; sv < (c >> 1); ++sv) { wait_full(sq + NHS + sv); release(sq + NHS + sv); }
+                const uint32_t seq = sq + NHS + (c >> 1);
                 const unsigned char* xsl = wait_full(seq) + t * 128;     // X rows (128 bytes each, 128-byte swizzle) at +0, Omega rows at +16 KB
+                sv = (c >> 1) + 1;
+                NMF_TRCW(TR_FULL, c);
                 wait(B_S0 + (j & 1)); tc_fence_after();
+                NMF_TRCW(TR_S, c);
                 const uint32_t zcol = lane_base + T_Z + 16 * NG * (j & 1) + 16 * grp;
                 const uint32_t ecol = lane_base + T_E + 32 * grp;
                 uint32_t s[16];
                 if (active) { tmem_ld16(zcol, s); tmem_wait_ld(); }
+                NMF_TRCW(TR_LD, c);
                 if (pending) { wait(B_G0 + grp); tc_fence_after(); }      // this group's E columns are free again
+                NMF_TRCW(TR_EFREE, c);
                 if (active) {
 #pragma unroll
                     for (int hf = 0; hf < 2; ++hf) {
@@ -668,16 +690,13 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                 tmem_wait_st();
                 tc_fence_before();
                 warp_arrive(B_P0 + grp);
+                NMF_TRCW(TR_HANDED, c);
                 pending = true;
             }
-            wait(B_G0 + grp);                            // this group's last AB of the tile is complete, and with it (the
-                                                         // tensor pipe completes in order) every MMA of the previous tile
-            if (tile + gridDim.x < g.n_tiles) {
-                if (HB == 1) wait(B_DONE);               // single buffer: every MMA of this tile must be complete
-                h0(sq + slots_per_tile, HB == 2 ? ((it + 1) & 1u) : 0u);
-            }
+            for (; sv < NSW; ++sv) { wait_full(sq + NHS + sv); release(sq + NHS + sv); }
+            wait(B_G0 + grp);                            // this group's last AB of the tile is complete
         }
-        wait(B_UPD);                                     // every MMA of the launch is complete
+        wait(B_DONE);                                    // every MMA of the last tile is complete
         tc_fence_after();
         // ---- accumulators -> this CTA's slab [2][128][KP] (grid.x <= n_tiles: every CTA had a tile); group g writes
         // the 16-column blocks g, g + NG, ... ----
@@ -695,6 +714,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             }
         }
     }
+    NMF_TRC_FLUSH(1);
     tc_fence_before();
     __syncthreads();
     if (warp == W_MMA) tmem_dealloc(tmem, 512);
@@ -743,16 +763,15 @@ inline int ng_of(int KP) { return KP <= 80 ? 4 : 2; }
 inline size_t smem_fixed_h(int NF, int KP, int NG) {
     return (size_t)3 * KP * NF * 2 + (size_t)(3 - npt_of(KP, NG, 2 * KP)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
 }
-inline size_t smem_fixed_w(int KP, int NG, int HB) {
-    return (size_t)(3 * HB + 3 - npt_of(KP, NG, 2 * KP)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
+inline size_t smem_fixed_w(int KP, int NG) {
+    return (size_t)(3 + 3 - npt_of(KP, NG, 2 * KP)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
 }
-inline int slots_for(size_t fixed, int slot_bytes) {
+// ring slots that fit beside `fixed` bytes, rounded down to a multiple of `mult` (see "Ring slots and groups")
+inline int slots_for(size_t fixed, int slot_bytes, int mult) {
     long long ns = ((long long)SMEM_MAX - (long long)fixed) / slot_bytes;
-    return (int)(ns > MAX_SLOTS ? MAX_SLOTS : ns);
+    if (ns > MAX_SLOTS) ns = MAX_SLOTS;
+    return ns < 0 ? 0 : (int)(ns / mult * mult);
 }
-// the H tile pieces are double-buffered in k_tc_w when at least three ring slots remain
-inline int hb_of(int KP, int NG) { return slots_for(smem_fixed_w(KP, NG, 2), SLOTW) >= 3 ? 2 : 1; }
-
 // the opt-in shared-memory size is a per-device function attribute: set once per device and instantiation
 template <typename Kern>
 cudaError_t set_smem_attr_once(Kern kern, bool (&done)[NMF_MAX_DEVICES], int device) {
@@ -801,9 +820,8 @@ int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, 
     h.W = w.W = W; h.H = w.H = H; w.slab = h.slab = reinterpret_cast<float*>(p->ws);
     h.N = w.N = rows; h.K = w.K = p->K; h.P = w.P = p->P; h.n_tiles = w.n_tiles = n_tiles;
     h.NF = w.NF = (rows + FCH - 1) / FCH * FCH; h.NC = w.NC = h.NF / FCH;
-    h.HB = w.HB = hb_of(KP, NG);
-    h.NS = slots_for(smem_fixed_h(h.NF, KP, NG), SLOT); w.NS = slots_for(smem_fixed_w(KP, NG, w.HB), SLOTW);
-    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 32, TILE, 0) &&
+    h.NS = slots_for(smem_fixed_h(h.NF, KP, NG), SLOT, NG); w.NS = slots_for(smem_fixed_w(KP, NG), SLOTW, 1);
+    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 64, TILE, 0) &&
               make_map(&w.mX, X, trows, p->P, 128, PSW, 128) && make_map(&w.mO, Om, trows, p->P, 128, PSW, 128);
     if (fit) ok = ok && make_map(&h.mH, H, (long long)batch * p->K, p->P, 16, TILE, 0) &&
                   make_map(&h.mX, X, trows, p->P, FCH, TILE, 0) && make_map(&h.mO, Om, trows, p->P, FCH, TILE, 0);
@@ -814,7 +832,7 @@ int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, 
     const int ctas_h = even_ctas(n_tiles, p->num_sms / batch);
     const int ctas_w = even_ctas(n_tiles, p->num_sms / (batch * MT));
     const size_t smem_h = smem_fixed_h(h.NF, KP, NG) + (size_t)h.NS * SLOT;
-    const size_t smem_w = smem_fixed_w(KP, NG, w.HB) + (size_t)w.NS * SLOTW;
+    const size_t smem_w = smem_fixed_w(KP, NG) + (size_t)w.NS * SLOTW;
     const int nk = rows * p->K;
     int rc = nmf_run_iterations(p, fit ? 40 : 41, X, Om, W, H, nullptr, rows, batch, iters, [&]() -> int {
         if (fit) {
@@ -838,7 +856,7 @@ void nmf_tcsplit_configure(nmf_plan* p) {
     if (p->K > 128 || p->N > 256) return;
     if (p->P + TILE >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
     const int KP = kp_of(p->K), NG = ng_of(KP), NF = (p->N + FCH - 1) / FCH * FCH;
-    if (slots_for(smem_fixed_h(NF, KP, NG), SLOT) < 2 || slots_for(smem_fixed_w(KP, NG, hb_of(KP, NG)), SLOTW) < 2) return;
+    if (slots_for(smem_fixed_h(NF, KP, NG), SLOT, NG) < NG || slots_for(smem_fixed_w(KP, NG), SLOTW, 1) < 2) return;
     p->s_ok = true;
 }
 
@@ -878,3 +896,29 @@ int nmf_tcsplit_project(nmf_plan* p, const float* H, const float* T, const float
     }
     return NMF_OK;
 }
+
+#ifdef NMF_TC_TRACE
+// trace build only (build.py build_trace): copies the event log of CTA (0, 0, 0) of the last split-kernel launches:
+// counts[2][18] events per kernel (k_tc_h, k_tc_w) and warp, events[2][18][2048] = event << 56 | argument << 48 | clock64
+extern "C" int nmf_debug_trace(unsigned int* counts_host, unsigned long long* events_host, int reset) {
+    if (cudaMemcpyFromSymbol(counts_host, tc::g_trace_n, sizeof(unsigned int) * tc::TRACE_KERNELS * tc::TRACE_WARPS) != cudaSuccess) return -1;
+    if (cudaMemcpyFromSymbol(events_host, tc::g_trace, sizeof(unsigned long long) * tc::TRACE_KERNELS * tc::TRACE_WARPS * tc::TRACE_LEN) != cudaSuccess) return -1;
+    if (reset) {
+        unsigned int z[tc::TRACE_KERNELS * tc::TRACE_WARPS] = {};
+        if (cudaMemcpyToSymbol(tc::g_trace_n, z, sizeof(z)) != cudaSuccess) return -1;
+    }
+    return tc::TRACE_LEN;
+}
+#endif
+
+#ifdef NMF_WAIT_DEBUG
+// debugging build only: copies the wait log of this translation unit (entries of 4 words) to `out_host`
+extern "C" int nmf_debug_wait_log(unsigned int* out_host, int max_entries) {
+    unsigned int n = 0;
+    if (cudaMemcpyFromSymbol(&n, tc::g_wait_log_n, sizeof(n)) != cudaSuccess) return -1;
+    if ((int)n > max_entries) n = max_entries;
+    if (n > 256) n = 256;
+    if (n && cudaMemcpyFromSymbol(out_host, tc::g_wait_log, n * 4 * sizeof(unsigned int)) != cudaSuccess) return -1;
+    return (int)n;
+}
+#endif
