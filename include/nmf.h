@@ -89,8 +89,9 @@ int nmf_plan_set_workspace(nmf_plan* plan, void* workspace_dev, size_t bytes);
 int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
 
 /* Select the kernel family of nmf_fit / nmf_fit_batched / nmf_project:
- *   0  automatic: the fastest family that covers the shape (a tensor-core family
- *      whenever K <= 128 and the operands fit shared memory, else FFMA)
+ *   0  automatic: the fastest family that covers the shape: the split tensor-core
+ *      kernels (4) whenever K <= 128 and the operands fit shared memory, else the
+ *      fused tensor-core kernel (3), else FFMA (2, 1)
  *   1  generic two-kernel FFMA path (any N <= 256, K <= 128; also what
  *      nmf_project runs when omega == NULL)
  *   2  fused FFMA per-pixel-tile kernel (K <= 50)

@@ -35,14 +35,15 @@ int check_ws(const nmf_plan* p) {
     return NMF_OK;
 }
 
-// 0 auto: fused tensor core (K <= 64) > split tensor core (K <= 128) > fused FFMA > generic
+// 0 auto: split tensor core (K <= 128; the fastest family on every measured shape) > fused tensor core (K <= 64) >
+// fused FFMA > generic
 int pick_variant(const nmf_plan* p) {
     if (p->variant_req == 1) return 1;
     if (p->variant_req == 2) return nmf_fused_available(p) ? 2 : 1;
-    if (p->variant_req == 4) return nmf_tcsplit_available(p) ? 4 : 1;
-    if (nmf_tc_available(p)) return 3;
-    if (p->variant_req == 3) return 1;
+    if (p->variant_req == 3) return nmf_tc_available(p) ? 3 : 1;
     if (nmf_tcsplit_available(p)) return 4;
+    if (p->variant_req == 4) return 1;
+    if (nmf_tc_available(p)) return 3;
     return nmf_fused_available(p) ? 2 : 1;
 }
 

@@ -53,6 +53,7 @@ constexpr int HS_SB = 16 * 128;            // Hs: bytes between 8-component grou
 constexpr int HS_BYTES = 8 * HS_SB;        // one BF16 piece of the H tile
 constexpr int SLOT = 16384;                // ring slot bytes
 constexpr int MAX_SLOTS = 8;
+constexpr int FLUSH_TILES = 16;            // tiles accumulated in TMEM between two flushes of A / B into the slab
 
 // TMEM columns (512 allocated).  A super-chunk is two chunks (32 frames / 32 pixels), one per group.
 constexpr uint32_t T_NUM = 0, T_DEN = 64;  // H phase: Num^T, Den^T [pixel][64]
@@ -205,8 +206,9 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
         constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
         const int NSC = (NC + 1) / 2;                    // H-phase super-chunks of 32 frames (the last may hold 16)
         constexpr int NSC2 = NCH2 / 2;                   // W-phase super-chunks of 32 pixels
-        uint32_t acc_started = 0;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+        uint32_t acc_started = 0, itm = 0;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, ++itm) {
+            if (itm % FLUSH_TILES == 0) acc_started = 0;         // the accumulators were flushed into the slab
             // ---- H phase ----
             auto issue_S = [&](int j) {                  // S(j): [128 px] x [32 frames], K = comps -> Z[j & 1]
                 if (elect_one()) {
@@ -342,7 +344,45 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             }
             tmem_wait_st();
         };
+        // The tensor cores accumulate in FP32 with truncation, so a long sum of positive terms comes out low and A, B do
+        // not lose exactly the same fraction: accumulated over all tiles of a CTA, W <- W A / B was biased by 3e-6 per
+        // iteration (8e-4 after 200 iterations at 200 x 1024^2, all of it in the scale split between W and H).  The
+        // accumulators are therefore added into the CTA's slab [2][N][KP] every FLUSH_TILES tiles and restarted.
+        // Group g handles M tile g; `add` = the slab already holds earlier flushes.
+        auto flush = [&](bool add) {
+            tc_fence_after();
+            if (grp < MT) {
+                const int fr = 128 * grp + t;
+                const bool fr_ok = fr < N;
+                float* sa = slab + (size_t)(fr_ok ? fr : 0) * KP;
+                float* sb = sa + (size_t)N * KP;
+#pragma unroll
+                for (int cg = 0; cg < 4; ++cg) {
+                    uint32_t a[16], bq[16];
+                    tmem_ld16(lane_base + T_ACC + 128 * grp + 16 * cg, a);       // warp-collective: no lane predicate
+                    tmem_ld16(lane_base + T_ACC + 128 * grp + 64 + 16 * cg, bq);
+                    tmem_wait_ld();
+                    if (fr_ok) {
+#pragma unroll
+                        for (int j = 0; j < 16; j += 4) {
+                            float4 va = make_float4(__uint_as_float(a[j]), __uint_as_float(a[j + 1]), __uint_as_float(a[j + 2]), __uint_as_float(a[j + 3]));
+                            float4 vb = make_float4(__uint_as_float(bq[j]), __uint_as_float(bq[j + 1]), __uint_as_float(bq[j + 2]), __uint_as_float(bq[j + 3]));
+                            float4* pa = reinterpret_cast<float4*>(sa + 16 * cg + j);
+                            float4* pb = reinterpret_cast<float4*>(sb + 16 * cg + j);
+                            if (add) {
+                                const float4 oa = *pa, ob = *pb;
+                                va.x += oa.x; va.y += oa.y; va.z += oa.z; va.w += oa.w;
+                                vb.x += ob.x; vb.y += ob.y; vb.z += ob.z; vb.w += ob.w;
+                            }
+                            *pa = va; *pb = vb;
+                        }
+                    }
+                }
+            }
+            tc_fence_before();
+        };
         uint32_t sq = 0;                                 // ring sequence number of this tile's first slot
+        uint32_t itl = 0;                                // tiles of this CTA done
         bool first = true;
         const int NSC = (NC + 1) / 2;
         constexpr int NSC2 = NCH2 / 2;
@@ -364,7 +404,10 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
                 split3_pair(h0, h1, hp1[j], hp2[j], hp3[j]);
             }
             if (!first) { wait(B_AB); }                  // every MMA of the previous tile is complete: Hs is free
+            if (!first && itl % FLUSH_TILES == 0) flush(itl > FLUSH_TILES);   // (the issuer restarts the accumulation with this
+                                                         // tile; it waits for B_HS, which follows the flush)
             first = false;
+            ++itl;
 #pragma unroll
             for (int gq = 0; gq < 4; ++gq) {
                 const uint32_t off = (t & 7) * 16 + (t >> 3) * 128 + (4 * grp + gq) * HS_SB;
@@ -513,29 +556,8 @@ k_tc_iter(const __grid_constant__ TcArgs g) {
             wait(B_ABG0 + grp);
         }
         wait(B_AB);                                      // every MMA of the last tile is complete
-        tc_fence_after();
-
-        // ---- the CTA's accumulators -> its slab [2][N][KP] (grid <= n_tiles: every CTA had a tile) ----
-        if (grp < MT) {
-            const int fr = 128 * grp + t;
-            const bool fr_ok = fr < N;
-            float* sa = slab + (size_t)(fr_ok ? fr : 0) * KP;
-            float* sb = sa + (size_t)N * KP;
-#pragma unroll
-            for (int cg = 0; cg < 4; ++cg) {
-                uint32_t a[16], bq[16];
-                tmem_ld16(lane_base + T_ACC + 128 * grp + 16 * cg, a);       // warp-collective: no lane predicate
-                tmem_ld16(lane_base + T_ACC + 128 * grp + 64 + 16 * cg, bq);
-                tmem_wait_ld();
-                if (fr_ok) {
-#pragma unroll
-                    for (int j = 0; j < 16; j += 4) {
-                        *reinterpret_cast<uint4*>(sa + 16 * cg + j) = make_uint4(a[j], a[j + 1], a[j + 2], a[j + 3]);
-                        *reinterpret_cast<uint4*>(sb + 16 * cg + j) = make_uint4(bq[j], bq[j + 1], bq[j + 2], bq[j + 3]);
-                    }
-                }
-            }
-        }
+        flush(itl > FLUSH_TILES);                        // what was accumulated since the last flush (grid <= n_tiles: every
+                                                         // CTA had a tile)
     }
     tc_fence_before();
     __syncthreads();

@@ -46,6 +46,7 @@ constexpr int PSW = 32;                   // k_tc_w: pixels per X / Omega ring s
 constexpr int SLOTW = 32768;              // k_tc_w ring slot: [128 frames][32 px] of X and of Omega, or [64 comps][128 px] of H
 constexpr int MAX_SLOTS = 12;
 constexpr int MAX_NG = 4;
+constexpr int FLUSH_TILES = 16;            // k_tc_w: tiles accumulated in TMEM between two flushes into the slab
 constexpr size_t SMEM_MAX = 227 * 1024;
 
 struct SplitArgs {
@@ -557,7 +558,9 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             __syncwarp();
         };
         bool acc_started = false;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x) {
+        uint32_t it = 0;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, ++it) {
+            if (it % FLUSH_TILES == 0) acc_started = false;      // the accumulators were flushed into the slab (see below)
             wait(B_HS);                                  // the tile's H pieces are in Hs
             NMF_TRCW(TR_M_HS, 0);
             issue_S2(0);
@@ -638,11 +641,42 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             warp_arrive(B_HS);
             NMF_TRCW(TR_H0_END, 0);
         };
-        uint32_t sq = 0;
-        bool first = true;
-        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile) {
-            if (!first) wait(B_DONE);                    // every MMA of the previous tile is complete: Hs is free
-            first = false;
+        // The tensor cores accumulate in FP32 with truncation: a sum of n positive terms comes out low by about n / 4
+        // ulp, and A and B do not lose exactly the same fraction.  Accumulated over all ~110 tiles of a CTA, W <- W A / B
+        // was biased by 1e-5 per iteration, the same sign for every component: after 200 iterations at 200 x 1024^2 W was
+        // 1.6e-3 too large and H 1.6e-3 too small against the fp64 oracle (their product, and the cost, agreed to 1e-6;
+        // the scale split between W and H is a neutral direction of Eq. 3 that nothing pulls back).  The accumulators are
+        // therefore added into the CTA's slab [2][128][KP] every FLUSH_TILES tiles (FP32 adds, round to nearest, in a
+        // fixed order) and restarted: the bias is proportional to the accumulation depth.  Group g handles the
+        // 16-column blocks g, g + NG, ...; `add` = the slab already holds earlier flushes.
+        auto flush = [&](bool add) {
+            tc_fence_after();
+            for (int cb = 16 * grp; cb < KP; cb += 16 * NG) {
+                uint32_t a[16], bq[16];
+                tmem_ld16(lane_base + T_ACC + cb, a);
+                tmem_ld16(lane_base + T_ACC + KP + cb, bq);
+                tmem_wait_ld();
+                float4* sa = reinterpret_cast<float4*>(slab + (size_t)t * KP + cb);
+                float4* sb = reinterpret_cast<float4*>(slab + (size_t)128 * KP + (size_t)t * KP + cb);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    float4 va = make_float4(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]));
+                    float4 vb = make_float4(__uint_as_float(bq[4 * j]), __uint_as_float(bq[4 * j + 1]), __uint_as_float(bq[4 * j + 2]), __uint_as_float(bq[4 * j + 3]));
+                    if (add) {
+                        const float4 oa = sa[j], ob = sb[j];
+                        va.x += oa.x; va.y += oa.y; va.z += oa.z; va.w += oa.w;
+                        vb.x += ob.x; vb.y += ob.y; vb.z += ob.z; vb.w += ob.w;
+                    }
+                    sa[j] = va; sb[j] = vb;
+                }
+            }
+            tc_fence_before();
+        };
+        uint32_t sq = 0, it = 0;
+        for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile, ++it) {
+            if (it > 0) wait(B_DONE);                    // every MMA of the previous tile is complete: Hs is free
+            if (it > 0 && it % FLUSH_TILES == 0) flush(it > FLUSH_TILES);    // (the MMA issuer restarts the accumulation
+                                                         // with this tile; it waits for B_HS, which follows the flush)
             h0(sq);
             // ---- steps: chunk c = NG j + grp of super-chunk j lies in ring slot c / 2 (32 pixels); the slots of the other
             // groups are only observed (waited for and released), in ring order; thread = (frame 128 m + t, 16 pixels),
@@ -697,22 +731,8 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             wait(B_G0 + grp);                            // this group's last AB of the tile is complete
         }
         wait(B_DONE);                                    // every MMA of the last tile is complete
-        tc_fence_after();
-        // ---- accumulators -> this CTA's slab [2][128][KP] (grid.x <= n_tiles: every CTA had a tile); group g writes
-        // the 16-column blocks g, g + NG, ... ----
-        for (int cb = 16 * grp; cb < KP; cb += 16 * NG) {
-            uint32_t a[16], bq[16];
-            tmem_ld16(lane_base + T_ACC + cb, a);
-            tmem_ld16(lane_base + T_ACC + KP + cb, bq);
-            tmem_wait_ld();
-            float* sa = slab + (size_t)t * KP + cb;
-            float* sb = sa + (size_t)128 * KP;
-#pragma unroll
-            for (int j = 0; j < 16; j += 4) {
-                *reinterpret_cast<uint4*>(sa + j) = make_uint4(a[j], a[j + 1], a[j + 2], a[j + 3]);
-                *reinterpret_cast<uint4*>(sb + j) = make_uint4(bq[j], bq[j + 1], bq[j + 2], bq[j + 3]);
-            }
-        }
+        flush(it > FLUSH_TILES);                         // what was accumulated since the last flush (grid.x <= n_tiles:
+                                                         // every CTA had a tile)
     }
     NMF_TRC_FLUSH(1);
     tc_fence_before();

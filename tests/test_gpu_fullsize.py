@@ -100,11 +100,12 @@ def test_component_sweep_full_size(stis_lib, K):
     print(f"sweep K={K} full size:", r)
 
 
-def test_stis_split_kernels_full_size(stis_lib):
-    """the split tensor-core kernels (variant 4) at the metric's shape, same stored oracle result"""
+def test_stis_fused_kernel_full_size(stis_lib):
+    """the one-kernel-per-iteration tensor-core variant (3) at the metric's shape, same stored oracle result (the
+    default is the split kernels, variant 4)"""
     g = _load("stis")
-    _, _, _, r = _check_fit(stis_lib, g, variant=4)
-    print("stis full size, split kernels:", r)
+    _, _, _, r = _check_fit(stis_lib, g, variant=3)
+    print("stis full size, fused kernel:", r)
 
 
 def test_survey_batch_full_size():

@@ -13,8 +13,7 @@ from gpu_util import (TOL_FACTOR, check_fit_parity, check_project_subtract_parit
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [1, 2, 0, 4]   # 1 = generic two-kernel path, 2 = fused FFMA, 0 = automatic (fused tensor-core kernel for K <= 64,
-                          # split tensor-core kernels for K <= 128), 4 = split tensor-core kernels
+VARIANTS = [1, 2, 3, 0]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), automatic (split tensor-core kernels, K <= 128)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)

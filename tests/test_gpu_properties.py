@@ -11,7 +11,7 @@ from paper_2309_04623_b200 import inputs, nmf
 from gpu_util import TOL_FACTOR, check_fit_parity, dev, gpu_fit, rel
 
 pytestmark = pytest.mark.gpu
-VARIANTS = [1, 2, 0, 4]   # generic, fused FFMA, automatic (fused tensor-core kernel when K <= 64), split tensor-core kernels
+VARIANTS = [1, 2, 3, 0]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), automatic (split tensor-core kernels, K <= 128)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -73,8 +73,8 @@ def test_ragged_and_extreme_shapes(variant, N, P, K):
     W0 = (0.1 + 0.9 * rng.random((N, K))).astype(np.float32)
     H0 = (0.1 + 0.9 * rng.random((K, P))).astype(np.float32)
     plan = nmf.Plan(N, P, K, variant=variant)
-    if variant == 4 and plan.variant != 4:
-        pytest.skip("W (3 BF16 pieces of NF x KP) + ring exceed shared memory: the split kernels stop short of N = 256 with K = 128")
+    if variant == 3 and plan.variant != 3:
+        pytest.skip("the fused tensor-core kernel stops at K = 64")
     Xd, Od, Wd, Hd = dev(X), dev(Om), dev(W0), dev(H0)
     plan.fit(Xd, Od, Wd, Hd, 8)
     torch.cuda.synchronize()
@@ -137,7 +137,7 @@ def test_host_entry_points_match_device_path():
     assert rel(C.numpy(), Co) <= TOL_FACTOR
 
 
-@pytest.mark.parametrize("variant", [0, 4])
+@pytest.mark.parametrize("variant", [3, 0])
 @pytest.mark.parametrize("N", [64, 96, 128, 200])
 def test_tensor_core_path_multi_tile_deterministic(N, variant):
     """Several pixel tiles per persistent CTA (the TMA ring wraps many times) with one and two 128-frame M tiles:
@@ -161,7 +161,33 @@ def test_tensor_core_path_multi_tile_deterministic(N, variant):
     assert rel(res[0][0], Wo) <= 1e-5 and rel(res[0][1], Ho) <= 1e-5
 
 
-@pytest.mark.parametrize("variant", [0, 4])
+@pytest.mark.parametrize("N,K,tiles", [(200, 100, 2), (200, 112, 3), (224, 100, 2), (240, 128, 2), (128, 100, 5), (200, 81, 4)])
+def test_split_kernels_small_rings(N, K, tiles):
+    """Large K with many frames leaves the split kernels two or three ring slots, and several tiles per persistent CTA
+    on all 148 SMs.  (N, K) = (200, 100) had three slots: a group that ran ahead of a late TMA load tested the mbarrier
+    parity of the slot's use before last, read a slot that had not landed and corrupted the transaction count --
+    launch failure, only with two or more tiles per CTA.)  Parity after 2 iterations, bitwise run-to-run equality."""
+    P = 128 * 148 * tiles
+    rng = np.random.default_rng(N + K)
+    X = (rng.random((N, P)) * 10).astype(np.float32)
+    Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.25)).astype(np.float32)
+    W0 = (0.1 + 0.9 * rng.random((N, K))).astype(np.float32)
+    H0 = (0.1 + 0.9 * rng.random((K, P))).astype(np.float32)
+    plan = nmf.Plan(N, P, K)
+    if plan.variant != 4:
+        pytest.skip("the operands of this shape do not fit the split kernels' shared memory")
+    res = []
+    for _ in range(2):
+        Wd, Hd = dev(W0), dev(H0)
+        plan.fit(dev(X), dev(Om), Wd, Hd, 2)
+        torch.cuda.synchronize()
+        res.append((Wd.cpu().numpy(), Hd.cpu().numpy()))
+    assert np.array_equal(res[0][0], res[1][0]) and np.array_equal(res[0][1], res[1][1])
+    Wo, Ho = orc.fit(X, Om, W0, H0, 2)
+    assert rel(res[0][0], Wo) <= TOL_FACTOR and rel(res[0][1], Ho) <= TOL_FACTOR
+
+
+@pytest.mark.parametrize("variant", [3, 0])
 def test_projection_many_targets(variant):
     """M = 300 science frames: the tensor-core projection handles them 256 at a time (two passes)."""
     N, P, K, M = 12, 2052, 9, 300
@@ -180,7 +206,32 @@ def test_projection_many_targets(variant):
     assert np.abs(out - outo).max() <= TOL_FACTOR * np.abs(T).max()
 
 
-@pytest.mark.parametrize("variant", [0, 4])
+@pytest.mark.parametrize("K,M", [(1, 600), (5, 4096), (13, 600), (13, 4096)])
+def test_generic_projection_many_targets_no_weights(K, M):
+    """omega == NULL projection runs the generic FFMA W half-step.  For K <= 13 its geometry allowed up to 1024 frames per
+    CTA and asked for up to 296 KB of shared memory (launch failure, coef overwritten from an unwritten slab): the frames
+    per CTA are now capped by the opt-in shared memory.  M up to the plan maximum of 4096."""
+    N, P = 8, 516
+    rng = np.random.default_rng(1000 * K + M)
+    H = (rng.random((K, P)) + 0.05).astype(np.float32)
+    T = (rng.random((M, P)) * 5).astype(np.float32)
+    C0 = (0.1 + 0.9 * rng.random((M, K))).astype(np.float32)
+    plan = nmf.Plan(N, P, K, max_targets=M)
+    C = dev(C0)
+    plan.project(dev(H), dev(T), None, C, 10)
+    torch.cuda.synchronize()
+    Co = orc.project(H, T, None, C0, 10)
+    assert rel(C.cpu().numpy(), Co) <= TOL_FACTOR
+    # the same through the generic family with weights (variant 1)
+    om = (rng.random((M, P)) * (rng.random((M, P)) > 0.2)).astype(np.float32)
+    plan1 = nmf.Plan(N, P, K, max_targets=M, variant=1)
+    C1 = dev(C0)
+    plan1.project(dev(H), dev(T), dev(om), C1, 10)
+    torch.cuda.synchronize()
+    assert rel(C1.cpu().numpy(), orc.project(H, T, om, C0, 10)) <= TOL_FACTOR
+
+
+@pytest.mark.parametrize("variant", [3, 0])
 def test_batched_more_problems_than_sms(variant):
     """160 independent small problems in one batched launch sequence (grid.y > number of SMs: the persistent
     CTAs of different problems are not co-resident and must not depend on one another)."""
