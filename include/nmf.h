@@ -91,7 +91,8 @@ int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
 /* Select the kernel family of nmf_fit / nmf_fit_batched / nmf_project:
  *   0  automatic: the fastest family that covers the shape: the split tensor-core
  *      kernels (4) whenever K <= 128 and the operands fit shared memory, else the
- *      fused tensor-core kernel (3), else FFMA (2, 1)
+ *      fused tensor-core kernel (3), else FFMA (2, 1); launch-bound problems of at most
+ *      64 pixel tiles (128 px) in all run the fused FFMA kernel (2)
  *   1  generic two-kernel FFMA path (any N <= 256, K <= 128; also what
  *      nmf_project runs when omega == NULL)
  *   2  fused FFMA per-pixel-tile kernel (K <= 50)

@@ -35,12 +35,14 @@ int check_ws(const nmf_plan* p) {
     return NMF_OK;
 }
 
-// 0 auto: split tensor core (K <= 128; the fastest family on every measured shape) > fused tensor core (K <= 64) >
-// fused FFMA > generic
+// 0 auto: split tensor core (K <= 128; the fastest family on every measured shape but the smallest) > fused tensor core
+// (K <= 64) > fused FFMA > generic.  Problems of at most 64 pixel tiles in all (tiny: 32) are launch-bound: there the
+// fused FFMA kernel (one light kernel + the update per iteration: 9.5 us against 13.6 us at tiny) comes first.
 int pick_variant(const nmf_plan* p) {
     if (p->variant_req == 1) return 1;
     if (p->variant_req == 2) return nmf_fused_available(p) ? 2 : 1;
     if (p->variant_req == 3) return nmf_tc_available(p) ? 3 : 1;
+    if (p->variant_req == 0 && nmf_fused_available(p) && (p->P + 127) / 128 * p->batch <= 64) return 2;
     if (nmf_tcsplit_available(p)) return 4;
     if (p->variant_req == 4) return 1;
     if (nmf_tc_available(p)) return 3;

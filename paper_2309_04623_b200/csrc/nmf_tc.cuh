@@ -210,17 +210,19 @@ __device__ __forceinline__ bool elect_one() {
 // exact 3-way BF16 split of two FP32 values, packed (low half = first value): x = x1 + x2 + x3 with
 // x1 = x rounded to 8 significant bits (half away from zero), x2 = the next 8 bits of the remainder (truncated),
 // x3 = what is left (at most 8 significant bits, so it is a BF16 number).  Integer / FADD / PRMT only: the
-// F2FP conversion pipe is a quarter-rate unit and was the limiter of the element-wise warps.
+// F2FP conversion pipe is a quarter-rate unit and was the limiter of the element-wise warps in round 1 (in round 2, with
+// 16 element-wise warps, piece 1 by one packed cvt.rn.bf16x2.f32 per pair -- two integer instructions fewer -- measured
+// the same as this form: the split arithmetic is not what bounds the kernels).
 __device__ __forceinline__ void split3_pair(float x0, float x1, uint32_t& p1, uint32_t& p2, uint32_t& p3) {
     const uint32_t a0 = (__float_as_uint(x0) + 0x8000u) & 0xffff0000u;
     const uint32_t a1 = (__float_as_uint(x1) + 0x8000u) & 0xffff0000u;
+    p1 = __byte_perm(a0, a1, 0x7632);
     const float r0 = x0 - __uint_as_float(a0);
     const float r1 = x1 - __uint_as_float(a1);
     const uint32_t b0 = __float_as_uint(r0) & 0xffff0000u;
     const uint32_t b1 = __float_as_uint(r1) & 0xffff0000u;
     const float s0 = r0 - __uint_as_float(b0);
     const float s1 = r1 - __uint_as_float(b1);
-    p1 = __byte_perm(a0, a1, 0x7632);
     p2 = __byte_perm(b0, b1, 0x7632);
     p3 = __byte_perm(__float_as_uint(s0), __float_as_uint(s1), 0x7632);
 }

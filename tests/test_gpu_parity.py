@@ -13,7 +13,7 @@ from gpu_util import (TOL_FACTOR, check_fit_parity, check_project_subtract_parit
 
 pytestmark = pytest.mark.gpu
 
-VARIANTS = [1, 2, 3, 0]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), automatic (split tensor-core kernels, K <= 128)
+VARIANTS = [1, 2, 3, 4]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), split tensor-core kernels (K <= 128; the automatic choice except for launch-bound sizes)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)

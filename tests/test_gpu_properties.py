@@ -11,7 +11,7 @@ from paper_2309_04623_b200 import inputs, nmf
 from gpu_util import TOL_FACTOR, check_fit_parity, dev, gpu_fit, rel
 
 pytestmark = pytest.mark.gpu
-VARIANTS = [1, 2, 3, 0]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), automatic (split tensor-core kernels, K <= 128)
+VARIANTS = [1, 2, 3, 4]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), split tensor-core kernels (K <= 128; the automatic choice except for launch-bound sizes)
 
 
 @pytest.mark.parametrize("variant", VARIANTS)
@@ -73,8 +73,8 @@ def test_ragged_and_extreme_shapes(variant, N, P, K):
     W0 = (0.1 + 0.9 * rng.random((N, K))).astype(np.float32)
     H0 = (0.1 + 0.9 * rng.random((K, P))).astype(np.float32)
     plan = nmf.Plan(N, P, K, variant=variant)
-    if variant == 3 and plan.variant != 3:
-        pytest.skip("the fused tensor-core kernel stops at K = 64")
+    if variant in (3, 4) and plan.variant != variant:
+        pytest.skip("the fused tensor-core kernel stops at K = 64; the split kernels' operands do not fit shared memory at N = 256, K = 128")
     Xd, Od, Wd, Hd = dev(X), dev(Om), dev(W0), dev(H0)
     plan.fit(Xd, Od, Wd, Hd, 8)
     torch.cuda.synchronize()
@@ -137,7 +137,7 @@ def test_host_entry_points_match_device_path():
     assert rel(C.numpy(), Co) <= TOL_FACTOR
 
 
-@pytest.mark.parametrize("variant", [3, 0])
+@pytest.mark.parametrize("variant", [3, 4])
 @pytest.mark.parametrize("N", [64, 96, 128, 200])
 def test_tensor_core_path_multi_tile_deterministic(N, variant):
     """Several pixel tiles per persistent CTA (the TMA ring wraps many times) with one and two 128-frame M tiles:
@@ -187,7 +187,7 @@ def test_split_kernels_small_rings(N, K, tiles):
     assert rel(res[0][0], Wo) <= TOL_FACTOR and rel(res[0][1], Ho) <= TOL_FACTOR
 
 
-@pytest.mark.parametrize("variant", [3, 0])
+@pytest.mark.parametrize("variant", [3, 4])
 def test_projection_many_targets(variant):
     """M = 300 science frames: the tensor-core projection handles them 256 at a time (two passes)."""
     N, P, K, M = 12, 2052, 9, 300
@@ -231,7 +231,7 @@ def test_generic_projection_many_targets_no_weights(K, M):
     assert rel(C1.cpu().numpy(), orc.project(H, T, om, C0, 10)) <= TOL_FACTOR
 
 
-@pytest.mark.parametrize("variant", [3, 0])
+@pytest.mark.parametrize("variant", [3, 4])
 def test_batched_more_problems_than_sms(variant):
     """160 independent small problems in one batched launch sequence (grid.y > number of SMs: the persistent
     CTAs of different problems are not co-resident and must not depend on one another)."""
@@ -249,3 +249,14 @@ def test_batched_more_problems_than_sms(variant):
     for b in (0, 1, 77, 147, 148, 159):
         Wo, Ho = orc.fit(X[b], Om[b], W0[b], H0[b], 6)
         assert rel(Wg[b], Wo) <= 1e-5 and rel(Hg[b], Ho) <= 1e-5, b
+
+
+def test_automatic_family_selection():
+    """variant 0: the split tensor-core kernels wherever they fit, the fused FFMA kernel for launch-bound sizes (at most 64
+    pixel tiles in all), the generic kernels where nothing else covers the shape"""
+    assert nmf.Plan(200, 1 << 20, 50).variant == 4
+    assert nmf.Plan(200, 1 << 20, 100).variant == 4
+    assert nmf.Plan(128, 65536, 20, batch=64).variant == 4
+    assert nmf.Plan(16, 4096, 5).variant == 2
+    assert nmf.Plan(16, 4096, 60).variant == 4          # no fused FFMA instantiation beyond K = 50
+    assert nmf.Plan(256, 1 << 16, 128).variant == 1
