@@ -162,9 +162,20 @@ int nmf_fit_tol(nmf_plan* plan, const float* X, const float* Omega, float* W, fl
 int nmf_objective(nmf_plan* plan, const float* X, const float* Omega, const float* W,
                   const float* H, double* out_host);
 
+/* Device staging of the two *_host calls below.  By default the library allocates
+ * it on first use (cudaMalloc, freed by nmf_plan_destroy) -- the one place where
+ * it allocates device memory on its own.  A caller who wants to own every device
+ * buffer hands over `bytes` >= nmf_plan_staging_bytes(plan, M) (M = largest number
+ * of science frames passed to nmf_project_subtract_host; 16-byte aligned; valid
+ * until the plan is destroyed or the staging is reset with (NULL, 0)); a *_host call
+ * that needs more than a caller-provided buffer holds returns NMF_ERR_WORKSPACE.
+ * Errors of set_staging: INVALID_ARG, ALIGNMENT.                                   */
+size_t nmf_plan_staging_bytes(const nmf_plan* plan, int M);
+int nmf_plan_set_staging(nmf_plan* plan, void* staging_dev, size_t bytes);
+
 /* End-to-end convenience for callers whose data lives in HOST memory: copies
- * X, Omega, W, H host->device into plan-owned staging buffers (allocated on
- * first use, freed by nmf_plan_destroy), runs nmf_fit, copies W and H back and
+ * X, Omega, W, H host->device into the staging buffer (see above), runs nmf_fit,
+ * copies W and H back and
  * SYNCHRONISES.  All four pointers are host pointers (pinned memory makes the
  * copies faster but is not required).  W, H are updated in place.                  */
 int nmf_fit_host(nmf_plan* plan, const float* X_host, const float* Omega_host, float* W_host,

@@ -69,6 +69,7 @@ int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
 
 int ensure_stage(nmf_plan* p, size_t bytes) {
     if (p->stage_bytes >= bytes) return NMF_OK;
+    if (p->stage_user) return NMF_ERR_WORKSPACE;         // a caller-provided staging buffer is never replaced behind the caller
     if (p->stage) { cudaFree(p->stage); p->stage = nullptr; p->stage_bytes = 0; }
     NMF_CUDA_TRY(p, cudaMalloc(&p->stage, bytes));
     p->stage_bytes = bytes;
@@ -125,6 +126,25 @@ int nmf_plan_set_workspace(nmf_plan* p, void* ws, size_t bytes) {
     return NMF_OK;
 }
 
+size_t nmf_plan_staging_bytes(const nmf_plan* p, int M) {
+    if (!p || M < 0) return 0;
+    const size_t np = nmf_align_up(sizeof(float) * (size_t)p->N * p->P, 256);
+    const size_t nk = nmf_align_up(sizeof(float) * (size_t)p->N * p->K, 256);
+    const size_t kp = nmf_align_up(sizeof(float) * (size_t)p->K * p->P, 256);
+    const size_t mp = nmf_align_up(sizeof(float) * (size_t)M * p->P, 256);
+    const size_t mk = nmf_align_up(sizeof(float) * (size_t)M * p->K, 256);
+    const size_t fit = 2 * np + nk + kp, proj = 3 * mp + mk;
+    return fit > proj ? fit : proj;
+}
+
+int nmf_plan_set_staging(nmf_plan* p, void* staging_dev, size_t bytes) {
+    if (!p || (staging_dev == nullptr) != (bytes == 0)) return NMF_ERR_INVALID_ARG;
+    if (staging_dev && misaligned(staging_dev)) return NMF_ERR_ALIGNMENT;
+    if (p->stage && !p->stage_user) cudaFree(p->stage);
+    p->stage = staging_dev; p->stage_bytes = bytes; p->stage_user = staging_dev != nullptr;
+    return NMF_OK;
+}
+
 int nmf_plan_set_stream(nmf_plan* p, void* s) {
     if (!p) return NMF_ERR_INVALID_ARG;
     p->stream = static_cast<cudaStream_t>(s);
@@ -144,7 +164,7 @@ int nmf_plan_get_variant(const nmf_plan* p) {
 
 int nmf_plan_destroy(nmf_plan* p) {
     if (!p) return NMF_ERR_INVALID_ARG;
-    if (p->stage) cudaFree(p->stage);
+    if (p->stage && !p->stage_user) cudaFree(p->stage);
     if (p->own_ws) cudaFree(p->own_ws);
     if (p->host_scratch) cudaFreeHost(p->host_scratch);
     if (p->g_exec) cudaGraphExecDestroy(p->g_exec);

@@ -43,6 +43,7 @@ struct nmf_plan {
     // host staging for the *_host entry points (plan-owned device buffers)
     void* stage = nullptr;
     size_t stage_bytes = 0;
+    bool stage_user = false;      // the staging buffer was handed over by the caller (nmf_plan_set_staging)
     void* own_ws = nullptr;       // workspace allocated by a *_host call when none was set
     double* host_scratch = nullptr;   // 8 pinned doubles: results read back by nmf_objective / nmf_fit_tol
     // iteration loop as a CUDA graph (nmf_run_iterations): one instantiated graph of `g_unroll` iterations, kept

@@ -22,7 +22,7 @@ LIB_PATH = os.path.join(_HERE, "libnmf_b200.so")
 
 SYMBOLS = (
     "nmf_plan_create", "nmf_plan_workspace_bytes", "nmf_plan_set_workspace", "nmf_plan_set_stream",
-    "nmf_plan_set_variant", "nmf_plan_get_variant", "nmf_plan_destroy", "nmf_fit", "nmf_fit_batched",
+    "nmf_plan_set_variant", "nmf_plan_get_variant", "nmf_plan_destroy", "nmf_plan_staging_bytes", "nmf_plan_set_staging", "nmf_fit", "nmf_fit_batched",
     "nmf_project", "nmf_subtract", "nmf_objective", "nmf_fit_host", "nmf_project_subtract_host",
     "nmf_ref_distance", "nmf_ref_select", "nmf_fit_tol", "nmf_derotate_stack",
     "nmf_plan_launch_count", "nmf_status_string", "nmf_plan_last_cuda_error",
@@ -50,6 +50,8 @@ def lib():
         L.nmf_plan_create.argtypes = [ctypes.POINTER(_vp), _ci, _cll, _ci, _ci, _ci]
         L.nmf_plan_workspace_bytes.argtypes = [_vp]; L.nmf_plan_workspace_bytes.restype = ctypes.c_size_t
         L.nmf_plan_set_workspace.argtypes = [_vp, _vp, ctypes.c_size_t]
+        L.nmf_plan_staging_bytes.argtypes = [_vp, _ci]; L.nmf_plan_staging_bytes.restype = ctypes.c_size_t
+        L.nmf_plan_set_staging.argtypes = [_vp, _vp, ctypes.c_size_t]
         L.nmf_plan_set_stream.argtypes = [_vp, _vp]
         L.nmf_plan_set_variant.argtypes = [_vp, _ci]
         L.nmf_plan_get_variant.argtypes = [_vp]
@@ -107,6 +109,13 @@ class Plan:
         self._check(lib().nmf_plan_set_workspace(self._h, self.workspace.data_ptr(), self.workspace.numel()))
         if variant:
             self._check(lib().nmf_plan_set_variant(self._h, variant))
+
+    def use_own_staging(self, M: int = 0):
+        """Allocate the staging of fit_host / project_subtract_host as a torch tensor owned by this object and hand it
+        to the library (nmf_plan_set_staging), so that the library allocates no device memory on its own."""
+        nbytes = lib().nmf_plan_staging_bytes(self._h, max(M, self.max_targets))
+        self.staging = torch.empty(nbytes, dtype=torch.uint8, device=self.device)
+        self._check(lib().nmf_plan_set_staging(self._h, self.staging.data_ptr(), nbytes))
 
     # -- plumbing ---------------------------------------------------------
     def _check(self, rc: int):

@@ -135,6 +135,19 @@ def test_host_entry_points_match_device_path():
     plan.project_subtract_host(dev(Hd), torch.from_numpy(p.T), torch.from_numpy(p.omega_t), C, out, 30)
     Co = orc.project(Hd, p.T, p.omega_t, p.C0, 30)
     assert rel(C.numpy(), Co) <= TOL_FACTOR
+    # the same with staging owned by the caller (nmf_plan_set_staging): bitwise the same results, and a staging buffer
+    # that is too small is refused instead of being replaced behind the caller
+    plan2 = nmf.Plan(p.N, p.P, p.K, max_targets=p.M)
+    plan2.use_own_staging(p.M)
+    W2, H2 = torch.from_numpy(p.W0.copy()), torch.from_numpy(p.H0.copy())
+    plan2.fit_host(torch.from_numpy(p.X), torch.from_numpy(p.Omega), W2, H2, 15)
+    assert np.array_equal(W2.numpy(), Wd) and np.array_equal(H2.numpy(), Hd)
+    L = nmf.lib()
+    small = torch.empty(1024, dtype=torch.uint8, device="cuda")
+    assert L.nmf_plan_set_staging(plan2._h, small.data_ptr(), 1024) == 0
+    assert L.nmf_fit_host(plan2._h, p.X.ctypes.data, p.Omega.ctypes.data, W2.data_ptr(), H2.data_ptr(), 1) == -4
+    assert L.nmf_plan_set_staging(plan2._h, None, 0) == 0
+    assert L.nmf_plan_set_staging(plan2._h, small.data_ptr(), 0) == -1
 
 
 @pytest.mark.parametrize("variant", [3, 4])
