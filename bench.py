@@ -406,8 +406,17 @@ def run_trace(args):
     plan.fit(X, Om, W, H, 1); torch.cuda.synchronize()
     L.nmf_debug_trace(counts, events, 1)
     names = {1: "slot landed", 2: "S ready", 3: "S loaded", 4: "piece columns free", 5: "chunk handed over",
-             6: "H pieces begin", 7: "H pieces done", 8: "update begin", 9: "update done",
-             16: "chunk ready", 17: "chunk MMAs issued", 18: "S series issued", 19: "H pieces ready"}
+             6: "H pieces begin", 7: "H pieces done", 8: "update begin", 9: "update done", 10: "previous tile's MMAs complete",
+             11: "H slot landed", 16: "chunk ready", 17: "chunk MMAs issued", 18: "S series issued", 19: "H pieces ready",
+             24: "ring slot acquired"}
+    if args.trace_raw:                                   # every event of every warp: kernel, warp, event, argument, clock64
+        with open(args.trace_raw, "w") as f:
+            f.write("kernel,warp,event,arg,clock\n")
+            for ki, kern in enumerate(("k_tc_h", "k_tc_w")):
+                for w in range(NW):
+                    for i in range(min(counts[ki * NW + w], LEN)):
+                        e = events[(ki * NW + w) * LEN + i]
+                        f.write(f"{kern},{w},{names.get((e >> 56) & 0xff, (e >> 56) & 0xff)},{(e >> 48) & 0xff},{e & 0xffffffffffff}\n")
     print(f"# Timeline of CTA (0,0,0), split tensor-core kernels, N={N} P={P} K={K} (cycles of clock64)\n")
     print("Command: `python bench.py --trace` (builds build/libnmf_trace.so with -DNMF_TC_TRACE; one fit iteration on random data)\n")
     for ki, kern in enumerate(("k_tc_h", "k_tc_w")):
@@ -429,10 +438,11 @@ def run_trace(args):
             gaps = {}
             for (e0, a0, t0), (e1, a1, t1) in zip(ev[len(ev) // 4:], ev[len(ev) // 4 + 1:]):     # skip the start-up quarter
                 gaps.setdefault((e0, e1), []).append(t1 - t0)
-            role = "MMA issuer" if any(e >= 16 for e, _, _ in ev) else f"element-wise, group {w // 4}, quadrant {w % 4}"
+            role = ("TMA producer" if any(e >= 24 for e, _, _ in ev) else "MMA issuer" if any(e >= 16 for e, _, _ in ev)
+                    else f"element-wise, group {w // 4}, quadrant {w % 4}")
             txt = "; ".join(f"{names.get(a, a)} -> {names.get(b, b)}: {sum(v) / len(v):.0f} x {len(v)}"
                             for (a, b), v in sorted(gaps.items(), key=lambda kv: -sum(kv[1]))[:8])
-            if w % 4 == 0 or role == "MMA issuer":
+            if w % 4 == 0 or not role.startswith("element"):
                 print(f"| {w} | {role} | {txt} |")
         print()
 
@@ -450,6 +460,7 @@ def main():
                     help="--impl reference: seconds of oracle steps allowed at full size before falling back to a crop")
     ap.add_argument("--configs", action="store_true", help="print the fit-iteration rate of every config and exit")
     ap.add_argument("--trace", action="store_true", help="print the tile timeline of the split tensor-core kernels (markdown) and exit")
+    ap.add_argument("--trace-raw", default="", help="with --trace: also write every recorded event to this CSV file")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     rank = int(os.environ.get("RANK", "0"))

@@ -112,9 +112,10 @@ __device__ __forceinline__ void trace_flush(int kern, int warp, int lane, unsign
 #endif
 // trace events: element-wise warps 1 slot landed, 2 S ready, 3 S loaded, 4 piece columns free, 5 pieces stored + chunk
 // handed over, 6 H pieces begin, 7 H pieces done, 8 update begin, 9 update done; MMA issuer 16 pieces of a chunk ready,
-// 17 its MMAs issued, 18 S series issued, 19 H pieces ready
-enum { TR_FULL = 1, TR_S, TR_LD, TR_EFREE, TR_HANDED, TR_H0_BEGIN, TR_H0_END, TR_UPD_BEGIN, TR_UPD_END,
-       TR_M_READY = 16, TR_M_ISSUED, TR_M_S, TR_M_HS };
+// 17 its MMAs issued, 18 S series issued, 19 H pieces ready; k_tc_w only: 10 previous tile's MMAs complete, 11 H slot
+// landed; TMA producer 24 ring slot acquired (argument = item of the tile)
+enum { TR_FULL = 1, TR_S, TR_LD, TR_EFREE, TR_HANDED, TR_H0_BEGIN, TR_H0_END, TR_UPD_BEGIN, TR_UPD_END, TR_TILE, TR_HSLOT,
+       TR_M_READY = 16, TR_M_ISSUED, TR_M_S, TR_M_HS, TR_T_ACQ = 24 };
 
 // ---------------------------------------------------------------- TMA (cp.async.bulk.tensor, 2-D tiled maps)
 // Loads the box of `tmap` whose first element is (x = innermost coordinate, y = row) into shared memory at

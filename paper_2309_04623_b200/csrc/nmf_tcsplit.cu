@@ -60,7 +60,7 @@ struct SplitArgs {
     int NS;                    // ring slots
 };
 
-enum { B_HS = 0, B_UPD, B_S0, B_S1, B_DONE, B_P0, B_G0 = B_P0 + MAX_NG, B_FULL = B_G0 + MAX_NG,
+enum { B_HS = 0, B_UPD, B_S0, B_S1, B_DONE, B_HSB, B_DONEB, B_HFULL, B_FRDY = B_HFULL + 4, B_FDONE, B_P0, B_G0 = B_P0 + MAX_NG, B_FULL = B_G0 + MAX_NG,
        B_EMPTY = B_FULL + MAX_SLOTS, B_COUNT = B_EMPTY + MAX_SLOTS };
 
 // piece pairs (a, b) of a product, small products first: a1b3 a3b1 a2b2 a1b2 a2b1 a1b1
@@ -519,10 +519,12 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
                 const int p0 = (int)(tile * TILE);
                 for (int h = 0; h < NHS; ++h) {
                     const uint32_t s = acquire(SLOTW);
+                    NMF_TRCW(TR_T_ACQ, h);
                     tma_load_2d(ring_s + s * SLOTW, &g.mH, p0, b * K + 64 * h, &bars[B_FULL + s]);
                 }
                 for (int c = 0; c < NSW; ++c) {
                     const uint32_t s = acquire(SLOTW);
+                    NMF_TRCW(TR_T_ACQ, NHS + c);
                     tma_load_2d(ring_s + s * SLOTW, &g.mX, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
                     tma_load_2d(ring_s + s * SLOTW + 128 * PSW * 4, &g.mO, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
                 }
@@ -623,6 +625,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
             NMF_TRCW(TR_H0_BEGIN, 0);
             for (int h = 0; h < NHS; ++h) {
                 const float* hsl = reinterpret_cast<const float*>(wait_full(sqt + h)) + t;
+                NMF_TRCW(TR_HSLOT, h);
                 for (int sb = grp; sb < 4; sb += NG) {
                     const int bi = 4 * h + sb;
                     if (bi < NBLK) {
@@ -675,6 +678,7 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
         uint32_t sq = 0, it = 0;
         for (long long tile = blockIdx.x; tile < g.n_tiles; tile += gridDim.x, sq += slots_per_tile, ++it) {
             if (it > 0) wait(B_DONE);                    // every MMA of the previous tile is complete: Hs is free
+            NMF_TRCW(TR_TILE, 0);
             if (it > 0 && it % FLUSH_TILES == 0) flush(it > FLUSH_TILES);    // (the MMA issuer restarts the accumulation
                                                          // with this tile; it waits for B_HS, which follows the flush)
             h0(sq);
@@ -741,6 +745,366 @@ k_tc_w(const __grid_constant__ SplitArgs g) {
 }
 
 // =====================================================================================================================
+// W half-step (and projection), K <= 64: the same stages as k_tc_w, software-pipelined ACROSS tiles.
+//
+// In k_tc_w a tile is a closed sequence -- H pieces, S', element-wise chunks, AB -- and the tensor pipe idles while the
+// next tile's H pieces are split and while the first chunks of a tile are computed (timeline: about 3 k of 9.5 k cycles
+// per tile).  Here the H pieces are double-buffered (Hs[tile & 1]) and the MMA issuer runs one continuous stream
+//     AB(t, chunks 0-3)  S'(t+1, 0)  AB(t, chunks 4-7)  S'(t+1, 1)  AB(t+1, chunks 0-3) ...
+// while every element-wise group does   chunk(t, g)  H pieces (pixels 0-63) of t+1  chunk(t, 4 + g)  H pieces (64-127) ...
+// The fp32 H' tile of tile t+1 does not pass through the ring: the TMA producer lands it, 64 pixels at a time, IN the
+// buffer Hs[(t+1) & 1] as soon as the MMAs of tile t-1 that read those pixels are complete (B_DONE, B_DONEB) -- a whole
+// tile before the pieces are needed; the element-wise warps read their values, meet at their group's named barrier and
+// overwrite them with the pieces.  The ring (four 32 KB slots at K > 32) then holds X and Omega only: one
+// full tile ahead.  The accumulators are flushed as in k_tc_w; around a flush the MMA issuer waits for the
+// element-wise warps (B_FRDY / B_FDONE), S' of the next tile is still issued ahead.
+// =====================================================================================================================
+template <int KS>
+__global__ void __launch_bounds__(32 * (4 * 4 + 2), 1)
+k_tc_wp(const __grid_constant__ SplitArgs g) {
+    constexpr int NG = 4;
+    constexpr int KP = 16 * KS;
+    constexpr int EW_WARPS = 4 * NG, W_MMA = EW_WARPS, W_TMA = EW_WARPS + 1;
+    constexpr int NPT = npt_of(KP, NG, 2 * KP);
+    static_assert(KS <= 4 && NPT == 3, "every piece of the M tile's rows of W lives in TMEM");
+    constexpr uint32_t T_WT = 0;                                          // piece i at i KP / 2
+    constexpr uint32_t T_Z = NPT * KP / 2, T_E = T_Z + 32 * NG;           // Z[jb] at T_Z + 16 NG jb, E[g] at T_E + 32 g
+    constexpr uint32_t T_ACC = 512 - 2 * KP;                              // A at T_ACC, B at T_ACC + KP
+    static_assert(T_E + 32 * NG <= T_ACC, "TMEM");
+    constexpr int NBLK = KP / 16;
+    constexpr int NSW = TILE / PSW;                      // X / Omega ring slots per tile
+    constexpr int HS_BYTES = (KP / 8) * HS_SB;           // one BF16 piece of the H tile
+    constexpr int HSBUF = 3 * HS_BYTES;                  // (the fp32 tile lands in the same buffer, see H0)
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int N = g.N, K = g.K;
+    unsigned char* ring = smem;
+    unsigned char* hs_p = ring + (size_t)g.NS * SLOTW;  // two buffers of 3 pieces of an H tile, [pixel][comp]
+    uint64_t* bars = reinterpret_cast<uint64_t*>(hs_p + 2 * HSBUF);
+    uint32_t* tptr = reinterpret_cast<uint32_t*>(bars + B_COUNT);
+    const RingCtl rc{(uint32_t)g.NS, 0xffffffffu / (uint32_t)g.NS + 1u};
+
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
+    const int b = blockIdx.y, m = blockIdx.z;
+    NMF_TRC_DECL;
+    const float* __restrict__ W = g.W + (size_t)b * N * K;
+    float* slab = g.slab + (((size_t)b * gridDim.z + m) * gridDim.x + blockIdx.x) * 2 * (size_t)128 * KP;
+    // tiles of this CTA: blockIdx.x, blockIdx.x + gridDim.x, ...  (gridDim.x <= n_tiles: at least one)
+    const uint32_t n_my = (uint32_t)((g.n_tiles - 1 - blockIdx.x) / gridDim.x) + 1u;
+
+    if (tid == 0) {
+        mbar_init(&bars[B_HS], EW_WARPS); mbar_init(&bars[B_HSB], EW_WARPS);
+        for (int i = 0; i < 4; ++i) mbar_init(&bars[B_HFULL + i], 1);
+        mbar_init(&bars[B_S0], 1); mbar_init(&bars[B_S1], 1); mbar_init(&bars[B_DONE], 1); mbar_init(&bars[B_DONEB], 1);
+        mbar_init(&bars[B_FRDY], 1); mbar_init(&bars[B_FDONE], EW_WARPS);
+        for (int i = 0; i < NG; ++i) { mbar_init(&bars[B_P0 + i], 4); mbar_init(&bars[B_G0 + i], 1); }
+        // every element-wise warp waits for and releases EVERY ring slot (see "Ring slots and groups")
+        for (int s = 0; s < g.NS; ++s) { mbar_init(&bars[B_FULL + s], 1); mbar_init(&bars[B_EMPTY + s], EW_WARPS); }
+        mbar_fence_init();
+    }
+    if (warp == W_MMA) tmem_alloc(tptr, 512);
+    if (warp == W_TMA && lane == 0) { tma_prefetch_desc(&g.mH); tma_prefetch_desc(&g.mX); tma_prefetch_desc(&g.mO); }
+    tc_fence_before();
+    __syncthreads();
+    tc_fence_after();
+    const uint32_t tmem = *tptr;
+    const uint32_t hs_s = smem_u32(hs_p), ring_s = smem_u32(ring);
+
+    if (warp < EW_WARPS) {
+        // the M tile's rows of W -> TMEM (A operand of S', fixed for the launch); lane = frame 128 m + t
+        const int q = warp & 3, grp = warp >> 2, t = 32 * q + lane;
+        const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
+        const int fr = 128 * m + t;
+        for (int bi = grp; bi < NBLK; bi += NG) {
+            uint32_t p[3][8];
+#pragma unroll
+            for (int j = 0; j < 8; ++j) {
+                const int k0 = 16 * bi + 2 * j;
+                const float w0 = (fr < N && k0 < K) ? W[(size_t)fr * K + k0] : 0.f;
+                const float w1 = (fr < N && k0 + 1 < K) ? W[(size_t)fr * K + k0 + 1] : 0.f;
+                split3_pair(w0, w1, p[0][j], p[1][j], p[2][j]);
+            }
+#pragma unroll
+            for (int i = 0; i < 3; ++i) tmem_st8(lane_base + T_WT + i * (KP / 2) + 8 * bi, p[i]);
+        }
+        tmem_wait_st();
+        tc_fence_before();
+    }
+    __syncthreads();
+    tc_fence_after();
+
+    if (warp == W_TMA) {
+        // =========================== TMA producer ===========================
+        // Per tile i, in the order in which they become possible: X / Omega slots 0, 1 of the tile; the first 64 pixels of
+        // the fp32 H' tile of tile i + 1 into Hs[(i + 1) & 1] (those rows are free once AB of chunks 0-3 of tile i - 1 is
+        // complete, B_DONE); slots 2, 3; the other 64 pixels (free after chunks 4-7 of tile i - 1, B_DONEB).
+        if (lane == 0) {
+            uint32_t seq = 0, ph_a = 0, ph_b = 0;
+            auto acquire = [&](uint32_t bytes) -> uint32_t {
+                uint32_t par;
+                const uint32_t s = rc.slot(seq, par);
+                mbar_wait(&bars[B_EMPTY + s], par ^ 1u);
+                mbar_expect_tx(&bars[B_FULL + s], bytes);
+                ++seq;
+                return s;
+            };
+            // half hf of the H' tile of tile i: rows 16 g + 4 r .. + 3 ([4 comps][64 px] = 1 KB) land where group g writes
+            // its part of piece r / 2 (see H0)
+            auto load_h = [&](uint32_t i, uint32_t hf) {
+                const int p0 = (int)((blockIdx.x + (long long)i * gridDim.x) * TILE) + 64 * (int)hf;
+                uint64_t* bar = &bars[B_HFULL + 2 * (i & 1u) + hf];
+                const uint32_t dst = hs_s + (i & 1u) * HSBUF + 1024 * hf;
+                mbar_expect_tx(bar, NBLK * 16 * 64 * 4);
+                for (int gb = 0; gb < NBLK; ++gb)
+#pragma unroll
+                    for (int r = 0; r < 4; ++r)
+                        tma_load_2d(dst + (r >> 1) * HS_BYTES + (2 * gb + (r & 1)) * HS_SB, &g.mH, p0, b * K + 16 * gb + 4 * r, bar);
+            };
+            auto load_x = [&](uint32_t i, int c) {
+                const int p0 = (int)((blockIdx.x + (long long)i * gridDim.x) * TILE);
+                const uint32_t s = acquire(SLOTW);
+                NMF_TRCW(TR_T_ACQ, 1 + c);
+                tma_load_2d(ring_s + s * SLOTW, &g.mX, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
+                tma_load_2d(ring_s + s * SLOTW + 128 * PSW * 4, &g.mO, p0 + PSW * c, b * N + 128 * m, &bars[B_FULL + s]);
+            };
+            load_h(0, 0); load_h(0, 1);
+            for (uint32_t i = 0; i < n_my; ++i) {
+                load_x(i, 0); load_x(i, 1);
+                if (i + 1 < n_my) {
+                    if (i >= 1) { mbar_wait(&bars[B_DONE], ph_a); ph_a ^= 1u; }        // chunks 0-3 of tile i - 1 are complete
+                    NMF_TRCW(TR_T_ACQ, 0);
+                    load_h(i + 1, 0);
+                }
+                load_x(i, 2); load_x(i, 3);
+                if (i + 1 < n_my) {
+                    if (i >= 1) { mbar_wait(&bars[B_DONEB], ph_b); ph_b ^= 1u; }       // chunks 4-7 of tile i - 1 are complete
+                    load_h(i + 1, 1);
+                }
+            }
+        }
+    } else if (warp == W_MMA) {
+        // =========================== MMA issuer ===========================
+        uint32_t ph = 0;
+        auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; tc_fence_after(); };
+        constexpr uint32_t id_s = idesc_bf16(128, 16 * NG, 0), id_ab = idesc_bf16(128, KP, 1);
+        uint64_t d_hs_k[3], d_hs_mn[3];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+            d_hs_k[i] = smem_desc(hs_s + i * HS_BYTES, HS_SB, 128);
+            d_hs_mn[i] = smem_desc(hs_s + i * HS_BYTES, 128, HS_SB);
+        }
+        constexpr uint32_t hs_kstep = (uint32_t)(2 * HS_SB) >> 4;
+        constexpr uint32_t hs_buf = (uint32_t)HSBUF >> 4;
+        auto issue_S2 = [&](uint32_t hb, int j) {        // S'(j): [128 frames] x [64 px], K = comps, from Hs[hb] -> Z[j]
+            if (elect_one()) {
+                const uint32_t boff = hb * hs_buf + ((uint32_t)(j * NG * 2 * 128) >> 4);
+                const uint32_t d = tmem + T_Z + 16 * NG * j;
+#pragma unroll
+                for (int pr = 0; pr < 6; ++pr)
+#pragma unroll
+                    for (int ks = 0; ks < KS; ++ks)
+                        mma16_ts(d, tmem + T_WT + PA[pr] * (KP / 2) + 8 * ks, d_hs_k[PB[pr]] + boff + ks * hs_kstep, id_s,
+                                 (pr | ks) ? 1u : 0u);
+                mma_commit(&bars[B_S0 + j]);
+            }
+            __syncwarp();
+        };
+        bool acc_started = false;
+        wait(B_HS);
+        NMF_TRCW(TR_M_HS, 0);
+        issue_S2(0, 0);
+        wait(B_HSB);
+        issue_S2(0, 1);
+        NMF_TRCW(TR_M_S, 1);
+        for (uint32_t it = 0; it < n_my; ++it) {
+            const uint32_t hb = it & 1u;
+            if (it % FLUSH_TILES == 0) {
+                acc_started = false;                     // the accumulators were flushed into the slab
+                if (it > 0) wait(B_FDONE);
+            }
+            for (int j = 0; j < 2; ++j) {
+                for (int gg = 0; gg < NG; ++gg) {
+                    const int c = NG * j + gg;
+                    wait(B_P0 + gg);
+                    NMF_TRCW(TR_M_READY, c);
+                    if (elect_one()) {
+                        const uint32_t boff = hb * hs_buf + ((uint32_t)(c * 2 * 128) >> 4);   // 16 pixels = 2 row groups
+                        const uint32_t z = tmem + T_Z + 16 * NG * j + 16 * gg, e = tmem + T_E + 32 * gg;
+                        const uint32_t a_q[3] = {e + O_Q1, e + O_Q2, e + O_Q3};
+                        const uint32_t a_r[3] = {z, z + 8, e + O_R3};
+#pragma unroll
+                        for (int pr = 0; pr < 6; ++pr) {
+                            const uint32_t acc = (acc_started || pr > 0) ? 1u : 0u;
+                            mma16_ts(tmem + T_ACC, a_q[PA[pr]], d_hs_mn[PB[pr]] + boff, id_ab, acc);
+                            mma16_ts(tmem + T_ACC + KP, a_r[PA[pr]], d_hs_mn[PB[pr]] + boff, id_ab, acc);
+                        }
+                        mma_commit(&bars[B_G0 + gg]);
+                    }
+                    __syncwarp();
+                    NMF_TRCW(TR_M_ISSUED, c);
+                    acc_started = true;
+                }
+                if (elect_one()) mma_commit(&bars[j ? B_DONEB : B_DONE]);   // pixels 64 j .. + 63 of Hs[hb] may be rewritten
+                __syncwarp();
+                if (it + 1 < n_my) {                     // the next tile's S'(j): Z[j] is free, its R pieces were read by
+                    wait(j ? B_HSB : B_HS);              // the MMAs just issued (the pipe is in order)
+                    NMF_TRCW(TR_M_HS, j);
+                    issue_S2(hb ^ 1u, j);
+                    NMF_TRCW(TR_M_S, j);
+                }
+            }
+            if ((it + 1) % FLUSH_TILES == 0 || it + 1 == n_my) {
+                if (elect_one()) mma_commit(&bars[B_FRDY]);
+                __syncwarp();
+            }
+        }
+    } else if (warp < EW_WARPS) {
+        // =========================== element-wise warps: group grp = warp / 4, lane quadrant q = warp % 4 ===========================
+        const int q = warp & 3, grp = warp >> 2;
+        const int t = 32 * q + lane;                     // TMEM lane = frame 128 m + t
+        const uint32_t lane_base = tmem + ((uint32_t)(32 * q) << 16);
+        const int fr = 128 * m + t;
+        const bool active = 128 * m + 32 * q < N;        // warp-uniform: some lane has a frame
+        uint32_t ph = 0;
+        auto wait = [&](int bar) { mbar_wait(&bars[bar], (ph >> bar) & 1u); ph ^= 1u << bar; };
+        auto wait_full = [&](uint32_t seq) -> const unsigned char* {
+            uint32_t par;
+            const uint32_t s = rc.slot(seq, par);
+            mbar_wait(&bars[B_FULL + s], par);
+            return ring + (size_t)s * SLOTW;
+        };
+        auto release = [&](uint32_t seq) {
+            __syncwarp();
+            uint32_t par;
+            if (lane == 0) mbar_arrive(&bars[B_EMPTY + rc.slot(seq, par)]);
+        };
+        auto warp_arrive = [&](int bar) {
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[bar]);
+        };
+        // H0, one half (64 pixels) of a tile at a time: the fp32 values of the H' tile that landed in Hs[hb] are replaced
+        // by the pieces Hs[hb][pixel][comp].  Group g takes the 16-component block g; thread = (pixel 64 hf + t % 64,
+        // components 8 (t / 64) .. + 7 of the block).  The fp32 rows of the block (four boxes of [4 comps][64 px], 1 KB
+        // each) lie exactly where group g writes its part of pieces 0 and 1, so a group only ever overwrites what its
+        // own threads have read: they read, meet at the group's named barrier, and write.
+        auto h0 = [&](uint32_t hb, uint32_t hf) {
+            NMF_TRCW(TR_H0_BEGIN, hf);
+            wait(B_HFULL + 2 * (int)hb + (int)hf);
+            NMF_TRCW(TR_HSLOT, hf);
+            if (grp < NBLK) {
+                const int kh = q >> 1, px = t & 63, kg = 2 * grp + kh;
+                unsigned char* buf = hs_p + (size_t)hb * HSBUF;
+                const unsigned char* land = buf + kh * HS_BYTES + 2 * grp * HS_SB + 1024 * hf + 4 * px;   // boxes r = 2 kh, 2 kh + 1
+                float h[8];
+#pragma unroll
+                for (int j = 0; j < 8; ++j) h[j] = *reinterpret_cast<const float*>(land + (j >> 2) * HS_SB + (j & 3) * 256);
+                if (8 * kg + 8 > K) {                    // rows at or beyond K hold another problem's data or zeros
+#pragma unroll
+                    for (int j = 0; j < 8; ++j) if (8 * kg + j >= K) h[j] = 0.f;
+                }
+                uint32_t p[3][4];
+#pragma unroll
+                for (int j = 0; j < 4; ++j) split3_pair(h[2 * j], h[2 * j + 1], p[0][j], p[1][j], p[2][j]);
+                asm volatile("bar.sync %0, 128;" ::"r"(1 + grp) : "memory");
+#pragma unroll
+                for (int i = 0; i < 3; ++i) st_piece_smem(buf + i * HS_BYTES, 64 * (int)hf + px, kg, p[i]);
+                fence_proxy_async();
+            }
+            warp_arrive(hf ? B_HSB : B_HS);
+            NMF_TRCW(TR_H0_END, hf);
+        };
+        auto flush = [&](bool add) {                     // see k_tc_w
+            tc_fence_after();
+            for (int cb = 16 * grp; cb < KP; cb += 16 * NG) {
+                uint32_t a[16], bq[16];
+                tmem_ld16(lane_base + T_ACC + cb, a);
+                tmem_ld16(lane_base + T_ACC + KP + cb, bq);
+                tmem_wait_ld();
+                float4* sa = reinterpret_cast<float4*>(slab + (size_t)t * KP + cb);
+                float4* sb = reinterpret_cast<float4*>(slab + (size_t)128 * KP + (size_t)t * KP + cb);
+#pragma unroll
+                for (int j = 0; j < 4; ++j) {
+                    float4 va = make_float4(__uint_as_float(a[4 * j]), __uint_as_float(a[4 * j + 1]), __uint_as_float(a[4 * j + 2]), __uint_as_float(a[4 * j + 3]));
+                    float4 vb = make_float4(__uint_as_float(bq[4 * j]), __uint_as_float(bq[4 * j + 1]), __uint_as_float(bq[4 * j + 2]), __uint_as_float(bq[4 * j + 3]));
+                    if (add) {
+                        const float4 oa = sa[j], ob = sb[j];
+                        va.x += oa.x; va.y += oa.y; va.z += oa.z; va.w += oa.w;
+                        vb.x += ob.x; vb.y += ob.y; vb.z += ob.z; vb.w += ob.w;
+                    }
+                    sa[j] = va; sb[j] = vb;
+                }
+            }
+            tc_fence_before();
+        };
+        h0(0, 0); h0(0, 1);
+        uint32_t sq = 0;
+        bool pending = false;
+        const int sw = t & 7;
+        for (uint32_t it = 0; it < n_my; ++it, sq += NSW) {
+            if (it > 0 && it % FLUSH_TILES == 0) {
+                wait(B_FRDY); flush(it > FLUSH_TILES);   // every MMA up to the previous tile is complete; the MMA issuer
+                warp_arrive(B_FDONE);                    // restarts the accumulation once every warp has flushed
+            }
+            // chunk c = NG j + grp lies in ring slot c / 2 (32 pixels); the slots of the other groups are only observed
+            // (waited for and released), in ring order; thread = (frame 128 m + t, 16 pixels), two halves of 8
+            int sv = 0;
+            for (int j = 0; j < 2; ++j) {
+                const int c = NG * j + grp;
+                for (; sv < (c >> 1); ++sv) { wait_full(sq + sv); release(sq + sv); }
+                const uint32_t seq = sq + (c >> 1);
+                const unsigned char* xsl = wait_full(seq) + t * 128;     // X rows (128 bytes each, 128-byte swizzle) at +0, Omega rows at +16 KB
+                sv = (c >> 1) + 1;
+                NMF_TRCW(TR_FULL, c);
+                wait(B_S0 + j); tc_fence_after();
+                NMF_TRCW(TR_S, c);
+                const uint32_t zcol = lane_base + T_Z + 16 * NG * j + 16 * grp;
+                const uint32_t ecol = lane_base + T_E + 32 * grp;
+                uint32_t s[16];
+                if (active) { tmem_ld16(zcol, s); tmem_wait_ld(); }
+                NMF_TRCW(TR_LD, c);
+                if (pending) { wait(B_G0 + grp); tc_fence_after(); }      // this group's E columns are free again
+                NMF_TRCW(TR_EFREE, c);
+                if (active) {
+#pragma unroll
+                    for (int hf = 0; hf < 2; ++hf) {
+                        float x[8], o[8];
+#pragma unroll
+                        for (int ch = 0; ch < 2; ++ch) {
+                            float4 xv = make_float4(0.f, 0.f, 0.f, 0.f), ov = xv;
+                            if (fr < N) {
+                                const int cs = ((4 * (c & 1) + 2 * hf + ch) ^ sw) << 4;
+                                xv = *reinterpret_cast<const float4*>(xsl + cs);
+                                ov = *reinterpret_cast<const float4*>(xsl + 128 * PSW * 4 + cs);
+                            }
+                            x[4 * ch] = xv.x; x[4 * ch + 1] = xv.y; x[4 * ch + 2] = xv.z; x[4 * ch + 3] = xv.w;
+                            o[4 * ch] = ov.x; o[4 * ch + 1] = ov.y; o[4 * ch + 2] = ov.z; o[4 * ch + 3] = ov.w;
+                        }
+                        Ew8 w;
+                        ew8(x, o, &s[8 * hf], w);
+                        ew8_store(zcol, ecol, hf, w);
+                    }
+                }
+                release(seq);                            // after the values were consumed
+                tmem_wait_st();
+                tc_fence_before();
+                warp_arrive(B_P0 + grp);
+                NMF_TRCW(TR_HANDED, c);
+                pending = true;
+                if (it + 1 < n_my) h0((it + 1) & 1u, (uint32_t)j);       // the next tile's H pieces, half j
+            }
+            for (; sv < NSW; ++sv) { wait_full(sq + sv); release(sq + sv); }
+        }
+        if (pending) wait(B_G0 + grp);
+        wait(B_FRDY);                                    // every MMA of the launch is complete
+        flush(n_my > FLUSH_TILES);
+    }
+    NMF_TRC_FLUSH(1);
+    tc_fence_before();
+    __syncthreads();
+    if (warp == W_MMA) tmem_dealloc(tmem, 512);
+}
+
+// =====================================================================================================================
 // fixed-order fp64 reduction of the slabs [B][MT][parts][2][128][KP] + W <- W o A / max(B, eps)      (a8)
 // 256 threads = 32 part lanes x 8 elements: lane q sums parts q, q + 32, ... in order, the 32 partial sums are then
 // added in lane order -- a fixed association, so the result is bitwise reproducible.
@@ -786,6 +1150,13 @@ inline size_t smem_fixed_h(int NF, int KP, int NG) {
 inline size_t smem_fixed_w(int KP, int NG) {
     return (size_t)(3 + 3 - npt_of(KP, NG, 2 * KP)) * (KP / 8) * HS_SB + B_COUNT * 8 + 16;
 }
+inline size_t smem_fixed_wp(int KP) { return (size_t)2 * 3 * (KP / 8) * HS_SB + B_COUNT * 8 + 16; }
+// Which W kernel: the pipelined one (k_tc_wp, K <= 64) wins where the element-wise load per tile is light -- the
+// projection of up to 64 frames (at most two of the four lane quadrants hold frames): 0.226 ms against 0.283 ms for 32
+// frames at 1024^2, K = 50.  With all 128 lanes busy (the fit) its MMAs and the element-wise warps run at the same time
+// and slow each other down -- 30 % more tensor-active cycles for the same MMAs -- and it is 5 % SLOWER than k_tc_w
+// (DESIGN.md 6.2), so the fit keeps k_tc_w.
+inline bool use_wp(int KP, bool fit, int rows) { return KP <= 64 && !fit && rows <= 64; }
 // ring slots that fit beside `fixed` bytes, rounded down to a multiple of `mult` (see "Ring slots and groups")
 inline int slots_for(size_t fixed, int slot_bytes, int mult) {
     long long ns = ((long long)SMEM_MAX - (long long)fixed) / slot_bytes;
@@ -816,6 +1187,18 @@ cudaError_t launch_w(const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st
     k_tc_w<KS, NG><<<grid, 32 * (4 * NG + 2), smem, st>>>(a);
     return cudaSuccess;
 }
+template <int KS>
+cudaError_t launch_wp(const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
+    static bool done[NMF_MAX_DEVICES] = {};
+    cudaError_t e = set_smem_attr_once(k_tc_wp<KS>, done, device);
+    if (e != cudaSuccess) return e;
+    k_tc_wp<KS><<<grid, 32 * (4 * 4 + 2), smem, st>>>(a);
+    return cudaSuccess;
+}
+inline cudaError_t launch_wp_ks(int KS, const SplitArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
+    return KS == 1 ? launch_wp<1>(a, grid, smem, st, device) : KS == 2 ? launch_wp<2>(a, grid, smem, st, device) :
+           KS == 3 ? launch_wp<3>(a, grid, smem, st, device) : launch_wp<4>(a, grid, smem, st, device);
+}
 // KS = 1 .. 5 (KP <= 80) run with four groups, KS = 6 .. 8 with two (ng_of)
 #define NMF_KS_SWITCH(fn, KS, ...)                                    \
     ((KS) == 1 ? fn<1, 4>(__VA_ARGS__) : (KS) == 2 ? fn<2, 4>(__VA_ARGS__) : (KS) == 3 ? fn<3, 4>(__VA_ARGS__) : \
@@ -840,8 +1223,10 @@ int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, 
     h.W = w.W = W; h.H = w.H = H; w.slab = h.slab = reinterpret_cast<float*>(p->ws);
     h.N = w.N = rows; h.K = w.K = p->K; h.P = w.P = p->P; h.n_tiles = w.n_tiles = n_tiles;
     h.NF = w.NF = (rows + FCH - 1) / FCH * FCH; h.NC = w.NC = h.NF / FCH;
-    h.NS = slots_for(smem_fixed_h(h.NF, KP, NG), SLOT, NG); w.NS = slots_for(smem_fixed_w(KP, NG), SLOTW, 1);
-    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, 64, TILE, 0) &&
+    const bool wp = use_wp(KP, fit, rows) && slots_for(smem_fixed_wp(KP), SLOTW, 1) >= 2;
+    const size_t fixed_w = wp ? smem_fixed_wp(KP) : smem_fixed_w(KP, NG);
+    h.NS = slots_for(smem_fixed_h(h.NF, KP, NG), SLOT, NG); w.NS = slots_for(fixed_w, SLOTW, 1);
+    bool ok = make_map(&w.mH, H, (long long)batch * p->K, p->P, wp ? 4 : 64, wp ? 64 : TILE, 0) &&
               make_map(&w.mX, X, trows, p->P, 128, PSW, 128) && make_map(&w.mO, Om, trows, p->P, 128, PSW, 128);
     if (fit) ok = ok && make_map(&h.mH, H, (long long)batch * p->K, p->P, 16, TILE, 0) &&
                   make_map(&h.mX, X, trows, p->P, FCH, TILE, 0) && make_map(&h.mO, Om, trows, p->P, FCH, TILE, 0);
@@ -852,14 +1237,15 @@ int split_run(nmf_plan* p, const float* X, const float* Om, float* W, float* H, 
     const int ctas_h = even_ctas(n_tiles, p->num_sms / batch);
     const int ctas_w = even_ctas(n_tiles, p->num_sms / (batch * MT));
     const size_t smem_h = smem_fixed_h(h.NF, KP, NG) + (size_t)h.NS * SLOT;
-    const size_t smem_w = smem_fixed_w(KP, NG) + (size_t)w.NS * SLOTW;
+    const size_t smem_w = fixed_w + (size_t)w.NS * SLOTW;
     const int nk = rows * p->K;
     int rc = nmf_run_iterations(p, fit ? 40 : 41, X, Om, W, H, nullptr, rows, batch, iters, [&]() -> int {
         if (fit) {
             NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_h, KS, h, dim3(ctas_h, batch), smem_h, p->stream, p->device));
             p->launches++;
         }
-        NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_w, KS, w, dim3(ctas_w, batch, MT), smem_w, p->stream, p->device));
+        if (wp) NMF_CUDA_TRY(p, launch_wp_ks(KS, w, dim3(ctas_w, batch, MT), smem_w, p->stream, p->device));
+        else NMF_CUDA_TRY(p, NMF_KS_SWITCH(launch_w, KS, w, dim3(ctas_w, batch, MT), smem_w, p->stream, p->device));
         k_w_update_split<<<dim3((nk + WU_E - 1) / WU_E, batch), WU_E * WU_Q, 0, p->stream>>>(w.slab, W, rows, p->K, KP, ctas_w, MT);
         p->launches += 2;
         return NMF_OK;
@@ -876,7 +1262,8 @@ void nmf_tcsplit_configure(nmf_plan* p) {
     if (p->K > 128 || p->N > 256) return;
     if (p->P + TILE >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
     const int KP = kp_of(p->K), NG = ng_of(KP), NF = (p->N + FCH - 1) / FCH * FCH;
-    if (slots_for(smem_fixed_h(NF, KP, NG), SLOT, NG) < NG || slots_for(smem_fixed_w(KP, NG), SLOTW, 1) < 2) return;
+    if (slots_for(smem_fixed_h(NF, KP, NG), SLOT, NG) < NG ||
+        slots_for(smem_fixed_w(KP, NG), SLOTW, 1) < 2) return;
     p->s_ok = true;
 }
 
