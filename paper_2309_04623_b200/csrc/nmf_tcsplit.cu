@@ -18,6 +18,9 @@
 //               the whole launch.  X and Omega rows are read only by the CTAs of their M tile; the ring is as deep
 //               as shared memory allows (the kernel waited for data, not for the tensor pipe).  Also the projection kernel (a9) with
 //               X = targets, Omega = omega, W = coef.
+//   k_tc_wp<KS>    the same stages software-pipelined across tiles (two buffers of H pieces, S' of the next tile queued
+//               behind AB of this one), K <= 64.  Used for projections of up to 64 frames, where it is 20 % faster; with
+//               all 128 lanes busy the overlapped MMAs run 30 % slower and it loses to k_tc_w (see use_wp).
 //   k_w_update_split   fixed-order fp64 reduction of the per-CTA slabs + W <- W o A / max(B, eps)  (a8)
 //
 // Ring slots and groups.  An mbarrier wait tests a phase PARITY, so a consumer may only test the "full" barrier of a

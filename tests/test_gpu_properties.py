@@ -219,6 +219,32 @@ def test_projection_many_targets(variant):
     assert np.abs(out - outo).max() <= TOL_FACTOR * np.abs(T).max()
 
 
+@pytest.mark.parametrize("M,P,K,iters", [
+    (1, 4, 1, 5), (31, 132, 16, 5), (33, 1028, 17, 5), (64, 4100, 33, 5), (32, 128 * 148 * 2 + 68, 50, 4),
+    (7, 128 * 148 * 3, 64, 3), (4, 128 * 148 * 17 + 192, 5, 3), (40, 128 * 148 * 33 + 64, 20, 2)])
+def test_projection_pipelined_kernel_shapes(M, P, K, iters):
+    """Projections of up to 64 frames with K <= 64 run the pipelined W kernel (k_tc_wp: H pieces double-buffered and
+    landed 64 pixels at a time, S' of the next tile queued behind AB): one tile, one to three tiles per CTA, ragged last
+    tile, more than 16 and more than 32 tiles per CTA (one and two accumulator flushes), every 16-component block count,
+    1 to 64 frames (one or two lane quadrants); twice, bitwise equal."""
+    rng = np.random.default_rng(100 * M + K)
+    H = (rng.random((K, P)) + 0.05).astype(np.float32)
+    T = (rng.random((M, P)) * 5).astype(np.float32)
+    om = (rng.random((M, P)) * (rng.random((M, P)) > 0.2)).astype(np.float32)
+    C0 = (0.1 + 0.9 * rng.random((M, K))).astype(np.float32)
+    plan = nmf.Plan(8, P, K, max_targets=M, variant=4)
+    Hd, Td, od = dev(H), dev(T), dev(om)
+    res = []
+    for _ in range(2):
+        C = dev(C0)
+        plan.project(Hd, Td, od, C, iters)
+        torch.cuda.synchronize()
+        res.append(C.cpu().numpy())
+    assert np.array_equal(res[0], res[1])
+    Co = orc.project(H, T, om, C0, iters)
+    assert rel(res[0], Co) <= TOL_FACTOR, rel(res[0], Co)
+
+
 @pytest.mark.parametrize("K,M", [(1, 600), (5, 4096), (13, 600), (13, 4096)])
 def test_generic_projection_many_targets_no_weights(K, M):
     """omega == NULL projection runs the generic FFMA W half-step.  For K <= 13 its geometry allowed up to 1024 frames per
