@@ -63,11 +63,14 @@ typedef enum nmf_status {
                                  forced variant (2, 3, 4) whose kernels do not cover the shape */
     NMF_ERR_WORKSPACE   = -4, /* workspace missing or smaller than nmf_plan_workspace_bytes  */
     NMF_ERR_ARCH        = -5, /* current device is not compute capability 10.x               */
-    NMF_ERR_CUDA        = -6  /* CUDA runtime / launch error (sticky until the plan is freed) */
+    NMF_ERR_CUDA        = -6, /* CUDA runtime / launch error (sticky until the plan is freed) */
+    NMF_ERR_STATIC_LIMIT = -7 /* nmf_objective_static: P > NMF_STATIC_MAX_P (its scratch has a
+                                 fixed size)                                                  */
 } nmf_status;
 
 #define NMF_MAX_N 256
 #define NMF_MAX_K 128
+#define NMF_STATIC_MAX_P 4194304LL /* 2048 x 2048 pixels: the limit of nmf_objective_static */
 
 typedef struct nmf_plan nmf_plan; /* opaque; owns host-side launch state only */
 
@@ -161,6 +164,25 @@ int nmf_fit_tol(nmf_plan* plan, const float* X, const float* Omega, float* W, fl
  * writes one double to host memory.                                               */
 int nmf_objective(nmf_plan* plan, const float* X, const float* Omega, const float* W,
                   const float* H, double* out_host);
+
+/* The same cost for callers that may not allocate (code under CUDA graph capture,
+ * tight serving loops, harnesses that forbid cudaMalloc): no plan, no workspace, and
+ * the call itself performs no cudaMalloc / cudaFree / cudaMallocHost -- its scratch
+ * (one fp64 partial sum per block of 128 pixels) is a fixed device array inside the
+ * library, 256 KB, held by every GPU that loads the library until the process exits.
+ *   X, Omega [N,P], W [N,K], H [K,P]   device, fp32, as for nmf_objective; read only
+ *   f_out_dev   device, out: ONE double, written in stream order (no host sync)
+ *   stream      cudaStream_t of the CURRENT device (NULL = default stream)
+ * Limit: P <= NMF_STATIC_MAX_P (2048^2 pixels), else NMF_ERR_STATIC_LIMIT and nothing
+ * is launched; N <= 256, K <= 128 as everywhere (UNSUPPORTED).
+ * Asynchronous.  Same kernels and summation order as nmf_objective: the result is
+ * bitwise the same.  The scratch is shared by ALL calls on a device and keeps the last
+ * call's contents; every element a call reads it has written first, so nothing is
+ * cleared -- but two calls that overlap on the GPU (different streams, no ordering
+ * between them) RACE on it: order them.  Errors: INVALID_ARG, UNSUPPORTED,
+ * STATIC_LIMIT, ARCH, CUDA (not sticky: there is no plan).                          */
+int nmf_objective_static(const float* X, const float* Omega, const float* W, const float* H,
+                         int N, long long P, int K, double* f_out_dev, void* stream);
 
 /* Device staging of the two *_host calls below.  By default the library allocates
  * it on first use (cudaMalloc, freed by nmf_plan_destroy) -- the one place where

@@ -334,6 +334,7 @@ const char* nmf_status_string(int code) {
         case NMF_ERR_WORKSPACE: return "NMF_ERR_WORKSPACE: workspace missing or too small";
         case NMF_ERR_ARCH: return "NMF_ERR_ARCH: device is not compute capability 10.x (B200)";
         case NMF_ERR_CUDA: return "NMF_ERR_CUDA: CUDA runtime or launch error";
+        case NMF_ERR_STATIC_LIMIT: return "NMF_ERR_STATIC_LIMIT: P beyond the fixed scratch of nmf_objective_static (NMF_STATIC_MAX_P = 2048^2 pixels)";
         default: return "unknown nmf status";
     }
 }

@@ -302,3 +302,60 @@ int nmf_aux_derotate_stack(nmf_plan* p, const float* R, const float* om, const f
     NMF_CUDA_TRY(p, cudaGetLastError());
     return NMF_OK;
 }
+
+// =====================================================================================================================
+// nmf_objective_static: the cost of Eq. 2 WITHOUT a plan, a workspace or any allocation (include/nmf.h).
+// The per-block partial sums of k_objective live in a file-scope device array of fixed size; every device that loads
+// the library holds it (256 KB) until the process exits.
+// =====================================================================================================================
+namespace {
+
+constexpr long long STATIC_MAX_BLOCKS = (NMF_STATIC_MAX_P + OBJ_THREADS - 1) / OBJ_THREADS;   // 32768 doubles = 256 KB
+constexpr size_t STATIC_MAX_SMEM = 200 * 1024;                                                 // as nmf_aux_objective_dev
+
+static __device__ __align__(256) double g_static_partial[STATIC_MAX_BLOCKS];
+
+// In host code `g_static_partial` is a host-side stand-in for the symbol, not a device address: the address the
+// kernels need comes from cudaGetSymbolAddress, once per device, with that device current.
+struct StaticDev { bool ready = false; double* partial = nullptr; };
+StaticDev g_static_dev[NMF_MAX_DEVICES];
+
+int static_setup(int device, double** partial) {
+    StaticDev& d = g_static_dev[device];
+    if (!d.ready) {                                       // (plain flag: the calls below are idempotent, a race repeats them)
+        int major = 0;
+        if (cudaDeviceGetAttribute(&major, cudaDevAttrComputeCapabilityMajor, device) != cudaSuccess) return NMF_ERR_CUDA;
+        if (major != 10) return NMF_ERR_ARCH;
+        double* ptr = nullptr;
+        if (cudaGetSymbolAddress(reinterpret_cast<void**>(&ptr), g_static_partial) != cudaSuccess || !ptr) return NMF_ERR_CUDA;
+        if (cudaFuncSetAttribute(k_objective, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)STATIC_MAX_SMEM) != cudaSuccess)
+            return NMF_ERR_CUDA;
+        d.partial = ptr;
+        d.ready = true;
+    }
+    *partial = d.partial;
+    return NMF_OK;
+}
+
+}  // namespace
+
+extern "C" int nmf_objective_static(const float* X, const float* Omega, const float* W, const float* H, int N, long long P,
+                                    int K, double* f_out_dev, void* stream) {
+    if (!X || !Omega || !W || !H || !f_out_dev || N < 1 || P < 1 || K < 1) return NMF_ERR_INVALID_ARG;
+    if (N > NMF_MAX_N || K > NMF_MAX_K) return NMF_ERR_UNSUPPORTED;
+    const size_t smem = sizeof(float) * ((size_t)N * K + (size_t)K * OBJ_THREADS);
+    if (P > NMF_STATIC_MAX_P || smem > STATIC_MAX_SMEM) return NMF_ERR_STATIC_LIMIT;
+    int device = 0;
+    if (cudaGetDevice(&device) != cudaSuccess) return NMF_ERR_CUDA;
+    if (device < 0 || device >= NMF_MAX_DEVICES) return NMF_ERR_UNSUPPORTED;
+    double* partial = nullptr;
+    const int rc = static_setup(device, &partial);
+    if (rc) return rc;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const unsigned grid = (unsigned)((P + OBJ_THREADS - 1) / OBJ_THREADS);
+    // every partial that is read (blocks 0 .. grid - 1) is written by this call's first kernel: nothing left over from
+    // an earlier call is read, so nothing needs clearing
+    k_objective<<<grid, OBJ_THREADS, smem, st>>>(X, Omega, W, H, partial, N, P, K);
+    k_objective_reduce<<<1, RED_THREADS, 0, st>>>(partial, (int)grid, f_out_dev);
+    return cudaGetLastError() == cudaSuccess ? NMF_OK : NMF_ERR_CUDA;
+}

@@ -25,7 +25,7 @@ SYMBOLS = (
     "nmf_plan_set_variant", "nmf_plan_get_variant", "nmf_plan_destroy", "nmf_plan_staging_bytes", "nmf_plan_set_staging", "nmf_fit", "nmf_fit_batched",
     "nmf_project", "nmf_subtract", "nmf_objective", "nmf_fit_host", "nmf_project_subtract_host",
     "nmf_ref_distance", "nmf_ref_select", "nmf_fit_tol", "nmf_derotate_stack",
-    "nmf_plan_launch_count", "nmf_status_string", "nmf_plan_last_cuda_error",
+    "nmf_plan_launch_count", "nmf_status_string", "nmf_plan_last_cuda_error", "nmf_objective_static",
 )
 
 _lib = None
@@ -71,6 +71,7 @@ def lib():
         L.nmf_plan_launch_count.argtypes = [_vp]; L.nmf_plan_launch_count.restype = _cll
         L.nmf_status_string.argtypes = [_ci]; L.nmf_status_string.restype = ctypes.c_char_p
         L.nmf_plan_last_cuda_error.argtypes = [_vp]; L.nmf_plan_last_cuda_error.restype = ctypes.c_char_p
+        L.nmf_objective_static.argtypes = [_vp, _vp, _vp, _vp, _ci, _cll, _ci, _vp, _vp]
         _lib = L
     return _lib
 
@@ -89,6 +90,24 @@ def _host(t: torch.Tensor, shape=None) -> int:
     if shape is not None and tuple(t.shape) != tuple(shape):
         raise ValueError(f"expected shape {tuple(shape)}, got {tuple(t.shape)}")
     return t.data_ptr()
+
+
+STATIC_MAX_P = 4194304      # NMF_STATIC_MAX_P of include/nmf.h
+
+
+def objective_static(X, Omega, W, H, out) -> None:
+    """nmf_objective_static: the cost of Eq. 2 into `out` (a float64 CUDA tensor of one element), enqueued on torch's
+    current stream of the tensors' device.  No plan, no workspace; the library call allocates nothing (its scratch is a
+    fixed 256 KB device array, P <= STATIC_MAX_P).  Calls that overlap on the GPU race on that scratch."""
+    N, P = X.shape
+    K = W.shape[1]
+    if not (isinstance(out, torch.Tensor) and out.is_cuda and out.dtype == torch.float64 and out.numel() == 1):
+        raise TypeError("expected a float64 CUDA tensor of one element")
+    with torch.cuda.device(X.device):
+        rc = lib().nmf_objective_static(_dev(X, (N, P)), _dev(Omega, (N, P)), _dev(W, (N, K)), _dev(H, (K, P)), N, P, K,
+                                        out.data_ptr(), torch.cuda.current_stream().cuda_stream)
+    if rc != 0:
+        raise NMFError(rc)
 
 
 class Plan:
