@@ -13,6 +13,8 @@ size_t plan_workspace(nmf_plan* p) {
     size_t t = nmf_tc_workspace(p);
     size_t ts = nmf_tcsplit_workspace(p);
     if (ts > t) t = ts;
+    size_t st = nmf_stream_workspace(p);
+    if (st > t) t = st;
     size_t sel = nmf_select_workspace(p);
     if (f > g) g = f;
     if (t > g) g = t;
@@ -37,12 +39,15 @@ int check_ws(const nmf_plan* p) {
 
 // 0 auto: split tensor core (K <= 128; the fastest family on every measured shape but the smallest) > fused tensor core
 // (K <= 64) > fused FFMA > generic.  Problems of at most 64 pixel tiles in all (tiny: 32) are launch-bound: there the
-// fused FFMA kernel (one light kernel + the update per iteration: 9.5 us against 13.6 us at tiny) comes first.
+// fused FFMA kernel (one light kernel + the update per iteration: 9.5 us against 13.6 us at tiny) comes first.  With
+// K <= 8 the streaming FP32 kernel (X, Omega once over HBM, no BF16 split) is faster than the tensor-core kernels.
 int pick_variant(const nmf_plan* p) {
     if (p->variant_req == 1) return 1;
+    if (p->variant_req == 5) return nmf_stream_available(p) ? 5 : 1;
     if (p->variant_req == 2) return nmf_fused_available(p) ? 2 : 1;
     if (p->variant_req == 3) return nmf_tc_available(p) ? 3 : 1;
     if (p->variant_req == 0 && nmf_fused_available(p) && (p->P + 127) / 128 * p->batch <= 64) return 2;
+    if (p->variant_req == 0 && nmf_stream_available(p)) return 5;
     if (nmf_tcsplit_available(p)) return 4;
     if (p->variant_req == 4) return 1;
     if (nmf_tc_available(p)) return 3;
@@ -60,7 +65,9 @@ int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
     if (p->variant_req == 2 && !nmf_fused_available(p)) return NMF_ERR_UNSUPPORTED;
     if (p->variant_req == 3 && !nmf_tc_available(p)) return NMF_ERR_UNSUPPORTED;
     if (p->variant_req == 4 && !nmf_tcsplit_available(p)) return NMF_ERR_UNSUPPORTED;
+    if (p->variant_req == 5 && !nmf_stream_available(p)) return NMF_ERR_UNSUPPORTED;
     const int v = pick_variant(p);
+    if (v == 5) return nmf_stream_fit(p, X, Om, W, H, iters, batch);
     if (v == 4) return nmf_tcsplit_fit(p, X, Om, W, H, iters, batch);
     if (v == 3) return nmf_tc_fit(p, X, Om, W, H, iters, batch);
     if (v == 2) return nmf_fused_fit(p, X, Om, W, H, iters, batch);
@@ -111,6 +118,7 @@ int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int ma
     nmf_fused_configure(p);
     nmf_tc_configure(p);
     nmf_tcsplit_configure(p);
+    nmf_stream_configure(p);
     p->ws_needed = plan_workspace(p);
     *out = p;
     return NMF_OK;
@@ -152,7 +160,7 @@ int nmf_plan_set_stream(nmf_plan* p, void* s) {
 }
 
 int nmf_plan_set_variant(nmf_plan* p, int v) {
-    if (!p || v < 0 || v > 4) return NMF_ERR_INVALID_ARG;
+    if (!p || v < 0 || v > 5) return NMF_ERR_INVALID_ARG;
     p->variant_req = v;
     return NMF_OK;
 }
@@ -192,7 +200,8 @@ int nmf_project(nmf_plan* p, const float* H, const float* T, const float* om, fl
     if (iters == 0) return NMF_OK;
     // tensor-core W phase with H fixed when the plan's fit runs there too (omega == NULL: generic path)
     if (om && pick_variant(p) == 3) return nmf_tc_project(p, H, T, om, C, M, iters);
-    if (om && pick_variant(p) == 4) return nmf_tcsplit_project(p, H, T, om, C, M, iters);
+    if (om && (pick_variant(p) == 4 || (pick_variant(p) == 5 && nmf_tcsplit_available(p))))   // (the streaming kernel is fit-only)
+        return nmf_tcsplit_project(p, H, T, om, C, M, iters);
     return nmf_generic_project(p, H, T, om, C, M, iters);
 }
 

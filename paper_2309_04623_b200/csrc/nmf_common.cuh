@@ -22,7 +22,7 @@ struct nmf_plan {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     size_t ws_needed = 0;
-    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core
+    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core, 5 streaming FP32
     long long launches = 0;
     int sticky = 0;               // first CUDA error seen (nmf_status)
     std::string cuda_msg;
@@ -40,6 +40,8 @@ struct nmf_plan {
     int t_ctas = 0;               // persistent CTAs per problem (0 = unavailable)
     // split tensor-core path (see nmf_tcsplit.cu)
     bool s_ok = false;
+    // streaming FP32 kernel for K <= 8 (see nmf_stream.cu)
+    bool st_ok = false;
     // host staging for the *_host entry points (plan-owned device buffers)
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -156,6 +158,12 @@ int    nmf_tcsplit_fit(nmf_plan* p, const float* X, const float* Om, float* W, f
                        int iters, int batch);
 int    nmf_tcsplit_project(nmf_plan* p, const float* H, const float* T, const float* om, float* C,
                            int M, int iters);
+// streaming FP32 kernel, one launch per iteration, K <= 8 (nmf_stream.cu)
+void   nmf_stream_configure(nmf_plan* p);
+size_t nmf_stream_workspace(const nmf_plan* p);
+bool   nmf_stream_available(const nmf_plan* p);
+int    nmf_stream_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
+                      int iters, int batch);
 // closest-frame reference selection (nmf_select.cu)
 size_t nmf_select_workspace(const nmf_plan* p);
 int    nmf_select_distance(nmf_plan* p, const float* T, const float* ot, const float* X, const float* Om,

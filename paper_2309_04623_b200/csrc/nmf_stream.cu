@@ -1,0 +1,307 @@
+// nmf_stream.cu -- one iteration of Eq. 3 for FEW components (K <= 8) as ONE streaming FP32 kernel.
+//
+// With K <= 8 an element (frame, pixel) costs 6K flops per half-step: less than the 13 instructions the tensor-core
+// kernels spend on splitting q and r into BF16 pieces, so the contractions stay on the FFMA pipe and the kernel is
+// bound by HBM: X and Omega cross it ONCE per iteration.  A persistent CTA (512 threads) takes pixel tiles of 32:
+// TMA lands the tile's [N frames][32 px] of X and of Omega (128-byte rows, 128-byte swizzle) and its [K][32 px] of H in
+// one of NS stages of shared memory, and both half-steps read them from there:
+//   H half-step (a1-a5)  lane = pixel, warp w takes frames w, w + 16, ...: s = W[n,:].h, q = Omega o x, r = Omega o s,
+//                        num += W[n,:] q, den += W[n,:] r; the 16 warps' partial sums are added in warp order through
+//                        shared memory; h' = h num / max(den, eps) -> global H and shared memory.
+//   W half-step (a6-a7)  thread = (frames j and j + ceil(N/2), 8 of the 32 pixels): s' = W[n,:].h', A[n,:] += q h',
+//                        B[n,:] += r' h' in registers over ALL tiles of the CTA; at the end the four threads of a
+//                        frame pair add up (shuffles) and write the CTA's slab [2][N][K].
+//   k_w_update_stream    fixed-order fp64 reduction of the slabs + W <- W o A / max(B, eps)   (a8)
+// Select semantics (entries with Omega == 0 never touch X), plain IEEE division: bitwise reproducible, exact under
+// power-of-two scaling.  Rows of a stage are addressed through the swizzle: 16-byte chunk c of row n lies at c ^ (n & 7).
+#include <cuda.h>
+#include "nmf_common.cuh"
+#include "nmf_tc.cuh"
+
+namespace {
+using namespace tc;
+
+constexpr int ST_THREADS = 512, ST_WARPS = 16, ST_PX = 32;
+constexpr int ST_MAXK = 8;
+constexpr int ST_MAX_STAGES = 4;
+constexpr size_t ST_SMEM_MAX = 227 * 1024;
+
+struct StreamArgs {
+    CUtensorMap mX, mO;        // X, Om [B*N, P]: box [N frames][32 px], 128-byte swizzle
+    CUtensorMap mH;            // H [B*K, P]: box [K][32 px]
+    const float* W; float* H; float* slab;
+    int N, NS; long long P; long long n_tiles;
+    int xbytes;                // bytes of one X (or Omega) box, rounded up to 1024
+    int stage_bytes;
+};
+
+__device__ __forceinline__ int swz(int n, int px) { return n * 128 + ((((px >> 2) ^ (n & 7)) << 4) | ((px & 3) << 2)); }
+
+template <int K>
+__global__ void __launch_bounds__(ST_THREADS, 1)
+k_stream(const __grid_constant__ StreamArgs g) {
+    constexpr int KP4 = (K + 3) / 4 * 4;
+    extern __shared__ __align__(1024) unsigned char smem[];
+    const int N = g.N, NH = (N + 1) / 2;
+    unsigned char* stages = smem;
+    float* Ws = reinterpret_cast<float*>(smem + (size_t)g.NS * g.stage_bytes);     // [N][KP4]
+    float* red = Ws + (size_t)N * KP4;                                             // [16 warps][2K][32]
+    float* hn = red + ST_WARPS * 2 * K * ST_PX;                                    // [K][32] new h
+    uint64_t* full = reinterpret_cast<uint64_t*>(hn + K * ST_PX);                  // [NS]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int b = blockIdx.y;
+    const float* __restrict__ Wg = g.W + (size_t)b * N * K;
+    float* __restrict__ Hg = g.H + (size_t)b * K * g.P;
+    const uint32_t n_my = (uint32_t)((g.n_tiles - 1 - blockIdx.x) / gridDim.x) + 1u;    // gridDim.x <= n_tiles
+    const uint32_t tx_bytes = (uint32_t)(2 * N * 128 + K * 128);
+
+    auto load_tile = [&](uint32_t i) {                   // thread 0: tile i of this CTA -> stage i % NS
+        const uint32_t s = i % (uint32_t)g.NS;
+        const int p0 = (int)((blockIdx.x + (long long)i * gridDim.x) * ST_PX);
+        const uint32_t dst = smem_u32(stages + (size_t)s * g.stage_bytes);
+        mbar_expect_tx(&full[s], tx_bytes);
+        tma_load_2d(dst, &g.mX, p0, b * N, &full[s]);
+        tma_load_2d(dst + g.xbytes, &g.mO, p0, b * N, &full[s]);
+        tma_load_2d(dst + 2 * g.xbytes, &g.mH, p0, b * K, &full[s]);
+    };
+    if (tid == 0) {
+        for (int s = 0; s < g.NS; ++s) mbar_init(&full[s], 1);
+        mbar_fence_init();
+        tma_prefetch_desc(&g.mX); tma_prefetch_desc(&g.mO); tma_prefetch_desc(&g.mH);
+    }
+    for (int i = tid; i < N * KP4; i += ST_THREADS) {
+        const int n = i / KP4, k = i - n * KP4;
+        Ws[i] = k < K ? Wg[(size_t)n * K + k] : 0.f;
+    }
+    __syncthreads();
+    if (tid == 0)
+        for (uint32_t i = 0; i < (uint32_t)g.NS && i < n_my; ++i) load_tile(i);
+
+    // W half-step roles: frame pair j = tid / 4 (frames j and j + NH), pixels 8 qd .. 8 qd + 7
+    const int j = tid >> 2, qd = tid & 3;
+    const int nA = j, nB = j + NH;
+    const bool okA = j < NH, okB = okA && nB < N;
+    float wA[K], wB[K], accA[2 * K], accB[2 * K];
+#pragma unroll
+    for (int k = 0; k < K; ++k) {
+        wA[k] = okA ? Ws[nA * KP4 + k] : 0.f;
+        wB[k] = okB ? Ws[nB * KP4 + k] : 0.f;
+        accA[k] = accA[K + k] = accB[k] = accB[K + k] = 0.f;
+    }
+
+    for (uint32_t it = 0; it < n_my; ++it) {
+        const uint32_t s = it % (uint32_t)g.NS;
+        const unsigned char* xs = stages + (size_t)s * g.stage_bytes;
+        const unsigned char* os = xs + g.xbytes;
+        const float* hs = reinterpret_cast<const float*>(xs + 2 * g.xbytes);      // [K][32]
+        const long long p0 = (blockIdx.x + (long long)it * gridDim.x) * ST_PX;
+        mbar_wait(&full[s], (it / (uint32_t)g.NS) & 1u);
+        // ---------------- H half-step: lane = pixel, frames warp, warp + 16, ... ----------------
+        {
+            float h[K], num[K], den[K];
+#pragma unroll
+            for (int k = 0; k < K; ++k) { h[k] = hs[k * ST_PX + lane]; num[k] = 0.f; den[k] = 0.f; }
+#pragma unroll 2
+            for (int n = warp; n < N; n += ST_WARPS) {
+                const int a = swz(n, lane);
+                const float x = *reinterpret_cast<const float*>(xs + a);
+                const float o = *reinterpret_cast<const float*>(os + a);
+                float w[KP4];
+#pragma unroll
+                for (int k4 = 0; k4 < KP4; k4 += 4) {
+                    const float4 v = *reinterpret_cast<const float4*>(Ws + n * KP4 + k4);
+                    w[k4] = v.x; w[k4 + 1] = v.y; w[k4 + 2] = v.z; w[k4 + 3] = v.w;
+                }
+                float sv = 0.f;
+#pragma unroll
+                for (int k = 0; k < K; ++k) sv = fmaf(w[k], h[k], sv);
+                const bool live = o > 0.f;
+                const float q = live ? o * x : 0.f, r = live ? o * sv : 0.f;
+#pragma unroll
+                for (int k = 0; k < K; ++k) { num[k] = fmaf(w[k], q, num[k]); den[k] = fmaf(w[k], r, den[k]); }
+            }
+#pragma unroll
+            for (int k = 0; k < K; ++k) {
+                red[(warp * 2 * K + k) * ST_PX + lane] = num[k];
+                red[(warp * 2 * K + K + k) * ST_PX + lane] = den[k];
+            }
+        }
+        __syncthreads();
+        if (tid < K * ST_PX) {                           // thread = (component k, pixel): warps in order
+            const int k = tid >> 5;
+            float num = 0.f, den = 0.f;
+#pragma unroll
+            for (int w = 0; w < ST_WARPS; ++w) {
+                num += red[(w * 2 * K + k) * ST_PX + lane];
+                den += red[(w * 2 * K + K + k) * ST_PX + lane];
+            }
+            const float hv = (hs[k * ST_PX + lane] * num) / fmaxf(den, NMF_EPS);
+            hn[k * ST_PX + lane] = hv;
+            if (p0 + lane < g.P) Hg[(size_t)k * g.P + p0 + lane] = hv;
+        }
+        __syncthreads();
+        // ---------------- W half-step: thread = (frames nA, nB; pixels 8 qd .. 8 qd + 7) ----------------
+        if (okA) {
+#pragma unroll
+            for (int i = 0; i < 2; ++i) {
+                const int c = 2 * qd + i;                // 16-byte chunk = 4 pixels
+                float4 h4[K];
+#pragma unroll
+                for (int k = 0; k < K; ++k) h4[k] = *reinterpret_cast<const float4*>(hn + k * ST_PX + 4 * c);
+                auto frame = [&](int n, const float (&w)[K], float (&acc)[2 * K]) {
+                    const int a = n * 128 + ((c ^ (n & 7)) << 4);
+                    const float4 x = *reinterpret_cast<const float4*>(xs + a);
+                    const float4 o = *reinterpret_cast<const float4*>(os + a);
+                    float4 sv = make_float4(0.f, 0.f, 0.f, 0.f);
+#pragma unroll
+                    for (int k = 0; k < K; ++k) {
+                        sv.x = fmaf(w[k], h4[k].x, sv.x); sv.y = fmaf(w[k], h4[k].y, sv.y);
+                        sv.z = fmaf(w[k], h4[k].z, sv.z); sv.w = fmaf(w[k], h4[k].w, sv.w);
+                    }
+                    float4 q, r;
+                    q.x = o.x > 0.f ? o.x * x.x : 0.f; r.x = o.x > 0.f ? o.x * sv.x : 0.f;
+                    q.y = o.y > 0.f ? o.y * x.y : 0.f; r.y = o.y > 0.f ? o.y * sv.y : 0.f;
+                    q.z = o.z > 0.f ? o.z * x.z : 0.f; r.z = o.z > 0.f ? o.z * sv.z : 0.f;
+                    q.w = o.w > 0.f ? o.w * x.w : 0.f; r.w = o.w > 0.f ? o.w * sv.w : 0.f;
+#pragma unroll
+                    for (int k = 0; k < K; ++k) {
+                        acc[k] = fmaf(q.x, h4[k].x, fmaf(q.y, h4[k].y, fmaf(q.z, h4[k].z, fmaf(q.w, h4[k].w, acc[k]))));
+                        acc[K + k] = fmaf(r.x, h4[k].x, fmaf(r.y, h4[k].y, fmaf(r.z, h4[k].z, fmaf(r.w, h4[k].w, acc[K + k]))));
+                    }
+                };
+                frame(nA, wA, accA);
+                if (okB) frame(nB, wB, accB);
+            }
+        }
+        __syncthreads();                                 // every thread is done with stage s (and with hn, red)
+        if (tid == 0 && it + (uint32_t)g.NS < n_my) load_tile(it + (uint32_t)g.NS);
+    }
+    // the four threads of a frame pair (adjacent lanes) add up, in a fixed order; lane qd == 0 writes the CTA's slab
+    float* slab = g.slab + ((size_t)b * gridDim.x + blockIdx.x) * 2 * (size_t)N * K;
+#pragma unroll
+    for (int k = 0; k < 2 * K; ++k) {
+        float a = accA[k], c = accB[k];
+        a += __shfl_xor_sync(0xffffffffu, a, 1); c += __shfl_xor_sync(0xffffffffu, c, 1);
+        a += __shfl_xor_sync(0xffffffffu, a, 2); c += __shfl_xor_sync(0xffffffffu, c, 2);
+        if (qd == 0) {
+            const int half = k / K, kk = k - half * K;
+            if (okA) slab[((size_t)half * N + nA) * K + kk] = a;
+            if (okB) slab[((size_t)half * N + nB) * K + kk] = c;
+        }
+    }
+}
+
+// fixed-order fp64 reduction of the slabs [B][parts][2][N][K] + W <- W o A / max(B, eps)      (a8)
+// 256 threads = 32 part lanes x 8 elements: lane q sums parts q, q + 32, ... in order, the 32 partial sums are then
+// added in lane order -- a fixed association, so the result is bitwise reproducible.
+constexpr int SU_E = 8, SU_Q = 32;
+__global__ void __launch_bounds__(SU_E * SU_Q)
+k_w_update_stream(const float* __restrict__ slab, float* __restrict__ W, int NK, int parts) {
+    __shared__ double sa[SU_Q][SU_E], sd[SU_Q][SU_E];
+    const int b = blockIdx.y;
+    const int e = threadIdx.x % SU_E, q = threadIdx.x / SU_E;
+    const int i = blockIdx.x * SU_E + e;
+    const bool ok = i < NK;
+    const size_t stride = (size_t)2 * NK;
+    const float* s = slab + (size_t)b * parts * stride + (ok ? i : 0);
+    double a = 0.0, d = 0.0;
+    if (ok) {
+#pragma unroll 5
+        for (int part = q; part < parts; part += SU_Q) {
+            a += (double)s[(size_t)part * stride];
+            d += (double)s[(size_t)part * stride + NK];
+        }
+    }
+    sa[q][e] = a; sd[q][e] = d;
+    __syncthreads();
+    if (q == 0 && ok) {
+#pragma unroll
+        for (int r = 1; r < SU_Q; ++r) { a += sa[r][e]; d += sd[r][e]; }
+        float* w = W + (size_t)b * NK + i;
+        *w = (*w * (float)a) / fmaxf((float)d, NMF_EPS);
+    }
+}
+
+// --------------------------------------------------------------------------------------------------------------------
+// host side
+// --------------------------------------------------------------------------------------------------------------------
+inline int xbytes_of(int N) { return (N * 128 + 1023) / 1024 * 1024; }
+inline int stage_bytes_of(int N, int K) { return (2 * xbytes_of(N) + K * 128 + 1023) / 1024 * 1024; }
+inline size_t fixed_bytes_of(int N, int K) {
+    const int KP4 = (K + 3) / 4 * 4;
+    return sizeof(float) * ((size_t)N * KP4 + (size_t)ST_WARPS * 2 * K * ST_PX + (size_t)K * ST_PX) + 8 * ST_MAX_STAGES + 16;
+}
+inline int stages_of(int N, int K) {
+    long long ns = ((long long)ST_SMEM_MAX - (long long)fixed_bytes_of(N, K)) / stage_bytes_of(N, K);
+    return ns > ST_MAX_STAGES ? ST_MAX_STAGES : ns < 0 ? 0 : (int)ns;
+}
+inline int ctas_of(const nmf_plan* p, int batch) {
+    const long long n_tiles = (p->P + ST_PX - 1) / ST_PX;
+    long long avail = p->num_sms / batch;
+    if (avail < 1) avail = 1;
+    if (avail > n_tiles) avail = n_tiles;
+    const long long per = (n_tiles + avail - 1) / avail;      // every CTA gets `per` or `per - 1` tiles
+    return (int)((n_tiles + per - 1) / per);
+}
+
+template <int K>
+cudaError_t launch_stream(const StreamArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
+    static bool done[NMF_MAX_DEVICES] = {};                   // the opt-in shared-memory size is a per-device attribute
+    if (!(device >= 0 && device < NMF_MAX_DEVICES && done[device])) {
+        cudaError_t e = cudaFuncSetAttribute(k_stream<K>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)ST_SMEM_MAX);
+        if (e != cudaSuccess) return e;
+        if (device >= 0 && device < NMF_MAX_DEVICES) done[device] = true;
+    }
+    k_stream<K><<<grid, ST_THREADS, smem, st>>>(a);
+    return cudaSuccess;
+}
+
+}  // namespace
+
+void nmf_stream_configure(nmf_plan* p) {
+    p->st_ok = false;
+    if (p->K > ST_MAXK || p->N > 256) return;
+    if (p->P + ST_PX >= (1LL << 31) || (long long)p->batch * p->N >= (1LL << 31)) return;   // TMA coordinates are int32
+    if (stages_of(p->N, p->K) < 2) return;
+    p->st_ok = true;
+}
+
+bool nmf_stream_available(const nmf_plan* p) { return p->st_ok; }
+
+size_t nmf_stream_workspace(const nmf_plan* p) {
+    if (!p->st_ok) return 0;
+    const size_t one = (size_t)ctas_of(p, 1) * 2 * p->N * p->K * sizeof(float);
+    const size_t all = (size_t)p->batch * ctas_of(p, p->batch) * 2 * p->N * p->K * sizeof(float);
+    return one > all ? one : all;
+}
+
+int nmf_stream_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
+    if (!p->st_ok) return NMF_ERR_UNSUPPORTED;
+    const int N = p->N, K = p->K;
+    StreamArgs a{};
+    a.W = W; a.H = H; a.slab = reinterpret_cast<float*>(p->ws);
+    a.N = N; a.P = p->P; a.n_tiles = (p->P + ST_PX - 1) / ST_PX;
+    a.NS = stages_of(N, K); a.xbytes = xbytes_of(N); a.stage_bytes = stage_bytes_of(N, K);
+    if (!(make_map(&a.mX, X, (long long)batch * N, p->P, N, ST_PX, 128) && make_map(&a.mO, Om, (long long)batch * N, p->P, N, ST_PX, 128) &&
+          make_map(&a.mH, H, (long long)batch * K, p->P, K, ST_PX, 0))) {
+        if (!p->sticky) { p->sticky = NMF_ERR_CUDA; p->cuda_msg = "cuTensorMapEncodeTiled failed"; }
+        return NMF_ERR_CUDA;
+    }
+    const int ctas = ctas_of(p, batch);
+    const size_t smem = (size_t)a.NS * a.stage_bytes + fixed_bytes_of(N, K);
+    const int nk = N * K;
+    int rc = nmf_run_iterations(p, 50, X, Om, W, H, nullptr, N, batch, iters, [&]() -> int {
+        const dim3 grid(ctas, batch);
+        cudaError_t e = K == 1 ? launch_stream<1>(a, grid, smem, p->stream, p->device) : K == 2 ? launch_stream<2>(a, grid, smem, p->stream, p->device) :
+                        K == 3 ? launch_stream<3>(a, grid, smem, p->stream, p->device) : K == 4 ? launch_stream<4>(a, grid, smem, p->stream, p->device) :
+                        K == 5 ? launch_stream<5>(a, grid, smem, p->stream, p->device) : K == 6 ? launch_stream<6>(a, grid, smem, p->stream, p->device) :
+                        K == 7 ? launch_stream<7>(a, grid, smem, p->stream, p->device) : launch_stream<8>(a, grid, smem, p->stream, p->device);
+        NMF_CUDA_TRY(p, e);
+        k_w_update_stream<<<dim3((nk + SU_E - 1) / SU_E, batch), SU_E * SU_Q, 0, p->stream>>>(a.slab, W, nk, ctas);
+        p->launches += 2;
+        return NMF_OK;
+    });
+    if (rc) return rc;
+    NMF_CUDA_TRY(p, cudaGetLastError());
+    return NMF_OK;
+}

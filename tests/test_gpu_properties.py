@@ -47,7 +47,7 @@ def test_mask_invariance_bitwise(variant, garbage):
     assert torch.isfinite(out).all() and bool((out[dev(q.omega_t) == 0] == -1.0).all())
 
 
-@pytest.mark.parametrize("variant", VARIANTS)
+@pytest.mark.parametrize("variant", VARIANTS + [5])
 def test_power_of_two_homogeneity_bitwise(variant):
     p = inputs.make_tiny()
     W1, H1, plan = gpu_fit(p, 30, variant)
@@ -82,6 +82,45 @@ def test_ragged_and_extreme_shapes(variant, N, P, K):
     Hg = Hd.cpu().numpy()
     assert rel(Wd.cpu().numpy(), Wo) <= TOL_FACTOR and rel(Hg, Ho) <= TOL_FACTOR
     assert np.all(Hg[:, P // 2] == 0.0)     # G4: fully masked column -> exactly 0
+
+
+@pytest.mark.parametrize("N,P,K,B", [(1, 4, 1, 1), (3, 36, 2, 1), (7, 132, 5, 1), (33, 1028, 7, 1), (129, 2052, 3, 1),
+                                     (200, 32 * 148 * 5 + 20, 5, 1), (256, 32 * 148 * 3 + 8, 8, 1), (200, 32 * 148 * 2, 1, 1),
+                                     (24, 2052, 6, 5), (12, 260, 4, 160)])
+def test_streaming_kernel_few_components(N, P, K, B):
+    """K <= 8 runs the streaming FP32 kernel (variant 5; the automatic choice there): K = 1 .. 8, N = 1 .. 256 (two to
+    four stages), ragged last tile, one tile to more tiles per CTA than stages, batched problems (more than SMs);
+    garbage where Omega == 0 and a repeated run must give bitwise the same factors."""
+    rng = np.random.default_rng(N * 1000 + K + B)
+    X = (rng.random((B, N, P)) * 10).astype(np.float32)
+    Om = (rng.random((B, N, P)) * (rng.random((B, N, P)) > 0.25)).astype(np.float32)
+    Om[:, :, P // 2] = 0         # one fully masked column
+    W0 = (0.1 + 0.9 * rng.random((B, N, K))).astype(np.float32)
+    H0 = (0.1 + 0.9 * rng.random((B, K, P))).astype(np.float32)
+    plan = nmf.Plan(N, P, K, batch=B)
+    assert plan.variant == 5 or (P + 127) // 128 * B <= 64       # launch-bound sizes take the fused FFMA kernel
+    plan = nmf.Plan(N, P, K, batch=B, variant=5)
+    assert plan.variant == 5
+    iters = 9                                                     # graph replay of 9 (>= 8) iterations
+    res = []
+    for garbage in (None, np.nan, 1e30):
+        Xg = X.copy()
+        if garbage is not None:
+            Xg[Om == 0] = garbage
+        Xd, Od, Wd, Hd = dev(Xg), dev(Om), dev(W0), dev(H0)
+        if B == 1:
+            plan.fit(Xd[0], Od[0], Wd[0], Hd[0], iters)
+        else:
+            plan.fit_batched(Xd, Od, Wd, Hd, iters)
+        torch.cuda.synchronize()
+        res.append((Wd.cpu().numpy(), Hd.cpu().numpy()))
+    for Wg, Hg in res[1:]:
+        assert np.array_equal(Wg, res[0][0]) and np.array_equal(Hg, res[0][1])
+    Wg, Hg = res[0]
+    for b in range(0, B, max(1, B // 4)):
+        Wo, Ho = orc.fit(X[b], Om[b], W0[b], H0[b], iters)
+        assert rel(Wg[b], Wo) <= TOL_FACTOR and rel(Hg[b], Ho) <= TOL_FACTOR, (b, rel(Wg[b], Wo), rel(Hg[b], Ho))
+        assert np.all(Hg[b][:, P // 2] == 0.0)
 
 
 def test_zero_entries_stay_zero_and_empty_iters():
