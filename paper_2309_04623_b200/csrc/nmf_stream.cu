@@ -21,7 +21,8 @@
 namespace {
 using namespace tc;
 
-constexpr int ST_THREADS = 512, ST_WARPS = 16, ST_PX = 32;
+constexpr int ST_GROUPS = 2, ST_GWARPS = 8, ST_GTHREADS = 32 * ST_GWARPS;       // two groups of eight compute warps
+constexpr int ST_CWARPS = ST_GROUPS * ST_GWARPS, ST_THREADS = 32 * (ST_CWARPS + 1), ST_PX = 32;   // + one TMA producer warp
 constexpr int ST_MAXK = 8;
 constexpr int ST_MAX_STAGES = 4;
 constexpr size_t ST_SMEM_MAX = 227 * 1024;
@@ -35,8 +36,11 @@ struct StreamArgs {
     int stage_bytes;
 };
 
-__device__ __forceinline__ int swz(int n, int px) { return n * 128 + ((((px >> 2) ^ (n & 7)) << 4) | ((px & 3) << 2)); }
-
+// Tiles alternate between the two groups (tile i of the CTA -> group i & 1), so that one group's H half-step overlaps
+// the other's W half-step; the stages form one ring filled by the producer warp.  An mbarrier wait tests a phase
+// PARITY: every compute warp therefore waits for EVERY tile's "full" barrier in ring order and arrives on its "empty"
+// barrier (count = all compute warps) -- for the other group's tiles without touching the data -- so no waiter is ever
+// two phases away from the barrier it tests.
 template <int K>
 __global__ void __launch_bounds__(ST_THREADS, 1)
 k_stream(const __grid_constant__ StreamArgs g) {
@@ -45,27 +49,20 @@ k_stream(const __grid_constant__ StreamArgs g) {
     const int N = g.N, NH = (N + 1) / 2;
     unsigned char* stages = smem;
     float* Ws = reinterpret_cast<float*>(smem + (size_t)g.NS * g.stage_bytes);     // [N][KP4]
-    float* red = Ws + (size_t)N * KP4;                                             // [16 warps][2K][32]
-    float* hn = red + ST_WARPS * 2 * K * ST_PX;                                    // [K][32] new h
-    uint64_t* full = reinterpret_cast<uint64_t*>(hn + K * ST_PX);                  // [NS]
-    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    float* red0 = Ws + (size_t)N * KP4;                                            // [group][8 warps][2K][32]
+    float* hn0 = red0 + ST_GROUPS * ST_GWARPS * 2 * K * ST_PX;                     // [group][K][32] new h
+    uint64_t* full = reinterpret_cast<uint64_t*>(hn0 + ST_GROUPS * K * ST_PX);     // [NS]
+    uint64_t* empty = full + ST_MAX_STAGES;                                        // [NS]
+    const int tid = threadIdx.x, lane = tid & 31;
+    const int warp = __shfl_sync(0xffffffffu, tid >> 5, 0);
     const int b = blockIdx.y;
     const float* __restrict__ Wg = g.W + (size_t)b * N * K;
     float* __restrict__ Hg = g.H + (size_t)b * K * g.P;
     const uint32_t n_my = (uint32_t)((g.n_tiles - 1 - blockIdx.x) / gridDim.x) + 1u;    // gridDim.x <= n_tiles
-    const uint32_t tx_bytes = (uint32_t)(2 * N * 128 + K * 128);
+    const uint32_t NS = (uint32_t)g.NS;
 
-    auto load_tile = [&](uint32_t i) {                   // thread 0: tile i of this CTA -> stage i % NS
-        const uint32_t s = i % (uint32_t)g.NS;
-        const int p0 = (int)((blockIdx.x + (long long)i * gridDim.x) * ST_PX);
-        const uint32_t dst = smem_u32(stages + (size_t)s * g.stage_bytes);
-        mbar_expect_tx(&full[s], tx_bytes);
-        tma_load_2d(dst, &g.mX, p0, b * N, &full[s]);
-        tma_load_2d(dst + g.xbytes, &g.mO, p0, b * N, &full[s]);
-        tma_load_2d(dst + 2 * g.xbytes, &g.mH, p0, b * K, &full[s]);
-    };
     if (tid == 0) {
-        for (int s = 0; s < g.NS; ++s) mbar_init(&full[s], 1);
+        for (uint32_t s = 0; s < NS; ++s) { mbar_init(&full[s], 1); mbar_init(&empty[s], ST_CWARPS); }
         mbar_fence_init();
         tma_prefetch_desc(&g.mX); tma_prefetch_desc(&g.mO); tma_prefetch_desc(&g.mH);
     }
@@ -74,11 +71,31 @@ k_stream(const __grid_constant__ StreamArgs g) {
         Ws[i] = k < K ? Wg[(size_t)n * K + k] : 0.f;
     }
     __syncthreads();
-    if (tid == 0)
-        for (uint32_t i = 0; i < (uint32_t)g.NS && i < n_my; ++i) load_tile(i);
 
-    // W half-step roles: frame pair j = tid / 4 (frames j and j + NH), pixels 8 qd .. 8 qd + 7
-    const int j = tid >> 2, qd = tid & 3;
+    if (warp == ST_CWARPS) {
+        // =========================== TMA producer ===========================
+        if (lane == 0) {
+            const uint32_t tx_bytes = (uint32_t)(2 * N * 128 + K * 128);
+            for (uint32_t i = 0; i < n_my; ++i) {
+                const uint32_t s = i % NS, u = i / NS;
+                if (u > 0) mbar_wait(&empty[s], (u - 1u) & 1u);
+                const int p0 = (int)((blockIdx.x + (long long)i * gridDim.x) * ST_PX);
+                const uint32_t dst = smem_u32(stages + (size_t)s * g.stage_bytes);
+                mbar_expect_tx(&full[s], tx_bytes);
+                tma_load_2d(dst, &g.mX, p0, b * N, &full[s]);
+                tma_load_2d(dst + g.xbytes, &g.mO, p0, b * N, &full[s]);
+                tma_load_2d(dst + 2 * g.xbytes, &g.mH, p0, b * K, &full[s]);
+            }
+        }
+        return;
+    }
+    // =========================== compute warps ===========================
+    const int grp = warp / ST_GWARPS, gw = warp - grp * ST_GWARPS, gt = tid - grp * ST_GTHREADS;
+    float* red = red0 + grp * ST_GWARPS * 2 * K * ST_PX;
+    float* hn = hn0 + grp * K * ST_PX;
+    auto group_sync = [&]() { asm volatile("bar.sync %0, %1;" ::"r"(1 + grp), "n"(ST_GTHREADS) : "memory"); };
+    // W half-step role: frame pair j = gt / 2 (frames j and j + NH), pixels 16 hf .. 16 hf + 15
+    const int j = gt >> 1, hf = gt & 1;
     const int nA = j, nB = j + NH;
     const bool okA = j < NH, okB = okA && nB < N;
     float wA[K], wB[K], accA[2 * K], accB[2 * K];
@@ -88,28 +105,37 @@ k_stream(const __grid_constant__ StreamArgs g) {
         wB[k] = okB ? Ws[nB * KP4 + k] : 0.f;
         accA[k] = accA[K + k] = accB[k] = accB[K + k] = 0.f;
     }
+    // H half-step role: lane = pixel, frames gw, gw + 8, ...: n & 7 == gw, so the swizzled column is fixed
+    const int hcol = (((lane >> 2) ^ gw) << 4) | ((lane & 3) << 2);
 
     for (uint32_t it = 0; it < n_my; ++it) {
-        const uint32_t s = it % (uint32_t)g.NS;
+        const uint32_t s = it % NS;
+        mbar_wait(&full[s], (it / NS) & 1u);
+        if ((int)(it & 1u) != grp) {                     // the other group's tile: observed only
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&empty[s]);
+            continue;
+        }
         const unsigned char* xs = stages + (size_t)s * g.stage_bytes;
         const unsigned char* os = xs + g.xbytes;
         const float* hs = reinterpret_cast<const float*>(xs + 2 * g.xbytes);      // [K][32]
         const long long p0 = (blockIdx.x + (long long)it * gridDim.x) * ST_PX;
-        mbar_wait(&full[s], (it / (uint32_t)g.NS) & 1u);
-        // ---------------- H half-step: lane = pixel, frames warp, warp + 16, ... ----------------
+        // ---------------- H half-step ----------------
         {
             float h[K], num[K], den[K];
 #pragma unroll
             for (int k = 0; k < K; ++k) { h[k] = hs[k * ST_PX + lane]; num[k] = 0.f; den[k] = 0.f; }
-#pragma unroll 2
-            for (int n = warp; n < N; n += ST_WARPS) {
-                const int a = swz(n, lane);
-                const float x = *reinterpret_cast<const float*>(xs + a);
-                const float o = *reinterpret_cast<const float*>(os + a);
+            const unsigned char* xr = xs + gw * 128 + hcol;
+            const unsigned char* orow = os + gw * 128 + hcol;
+            const float* wr = Ws + gw * KP4;
+#pragma unroll 4
+            for (int n = gw; n < N; n += ST_GWARPS, xr += ST_GWARPS * 128, orow += ST_GWARPS * 128, wr += ST_GWARPS * KP4) {
+                const float x = *reinterpret_cast<const float*>(xr);
+                const float o = *reinterpret_cast<const float*>(orow);
                 float w[KP4];
 #pragma unroll
                 for (int k4 = 0; k4 < KP4; k4 += 4) {
-                    const float4 v = *reinterpret_cast<const float4*>(Ws + n * KP4 + k4);
+                    const float4 v = *reinterpret_cast<const float4*>(wr + k4);
                     w[k4] = v.x; w[k4 + 1] = v.y; w[k4 + 2] = v.z; w[k4 + 3] = v.w;
                 }
                 float sv = 0.f;
@@ -122,16 +148,16 @@ k_stream(const __grid_constant__ StreamArgs g) {
             }
 #pragma unroll
             for (int k = 0; k < K; ++k) {
-                red[(warp * 2 * K + k) * ST_PX + lane] = num[k];
-                red[(warp * 2 * K + K + k) * ST_PX + lane] = den[k];
+                red[(gw * 2 * K + k) * ST_PX + lane] = num[k];
+                red[(gw * 2 * K + K + k) * ST_PX + lane] = den[k];
             }
         }
-        __syncthreads();
-        if (tid < K * ST_PX) {                           // thread = (component k, pixel): warps in order
-            const int k = tid >> 5;
+        group_sync();
+        if (gt < K * ST_PX) {                            // thread = (component k, pixel): the group's warps in order
+            const int k = gt >> 5;
             float num = 0.f, den = 0.f;
 #pragma unroll
-            for (int w = 0; w < ST_WARPS; ++w) {
+            for (int w = 0; w < ST_GWARPS; ++w) {
                 num += red[(w * 2 * K + k) * ST_PX + lane];
                 den += red[(w * 2 * K + K + k) * ST_PX + lane];
             }
@@ -139,12 +165,12 @@ k_stream(const __grid_constant__ StreamArgs g) {
             hn[k * ST_PX + lane] = hv;
             if (p0 + lane < g.P) Hg[(size_t)k * g.P + p0 + lane] = hv;
         }
-        __syncthreads();
-        // ---------------- W half-step: thread = (frames nA, nB; pixels 8 qd .. 8 qd + 7) ----------------
+        group_sync();
+        // ---------------- W half-step: thread = (frames nA, nB; pixels 16 hf .. 16 hf + 15) ----------------
         if (okA) {
 #pragma unroll
-            for (int i = 0; i < 2; ++i) {
-                const int c = 2 * qd + i;                // 16-byte chunk = 4 pixels
+            for (int i = 0; i < 4; ++i) {
+                const int c = 4 * hf + i;                // 16-byte chunk = 4 pixels
                 float4 h4[K];
 #pragma unroll
                 for (int k = 0; k < K; ++k) h4[k] = *reinterpret_cast<const float4*>(hn + k * ST_PX + 4 * c);
@@ -173,17 +199,16 @@ k_stream(const __grid_constant__ StreamArgs g) {
                 if (okB) frame(nB, wB, accB);
             }
         }
-        __syncthreads();                                 // every thread is done with stage s (and with hn, red)
-        if (tid == 0 && it + (uint32_t)g.NS < n_my) load_tile(it + (uint32_t)g.NS);
+        group_sync();                                    // the group is done with the stage (and with hn, red)
+        if (lane == 0) mbar_arrive(&empty[s]);
     }
-    // the four threads of a frame pair (adjacent lanes) add up, in a fixed order; lane qd == 0 writes the CTA's slab
-    float* slab = g.slab + ((size_t)b * gridDim.x + blockIdx.x) * 2 * (size_t)N * K;
+    // the two threads of a frame pair (adjacent lanes) add up; lane hf == 0 writes the group's slab (part 2 cta + group)
+    float* slab = g.slab + (((size_t)b * gridDim.x + blockIdx.x) * ST_GROUPS + grp) * 2 * (size_t)N * K;
 #pragma unroll
     for (int k = 0; k < 2 * K; ++k) {
         float a = accA[k], c = accB[k];
         a += __shfl_xor_sync(0xffffffffu, a, 1); c += __shfl_xor_sync(0xffffffffu, c, 1);
-        a += __shfl_xor_sync(0xffffffffu, a, 2); c += __shfl_xor_sync(0xffffffffu, c, 2);
-        if (qd == 0) {
+        if (hf == 0) {
             const int half = k / K, kk = k - half * K;
             if (okA) slab[((size_t)half * N + nA) * K + kk] = a;
             if (okB) slab[((size_t)half * N + nB) * K + kk] = c;
@@ -229,7 +254,7 @@ inline int xbytes_of(int N) { return (N * 128 + 1023) / 1024 * 1024; }
 inline int stage_bytes_of(int N, int K) { return (2 * xbytes_of(N) + K * 128 + 1023) / 1024 * 1024; }
 inline size_t fixed_bytes_of(int N, int K) {
     const int KP4 = (K + 3) / 4 * 4;
-    return sizeof(float) * ((size_t)N * KP4 + (size_t)ST_WARPS * 2 * K * ST_PX + (size_t)K * ST_PX) + 8 * ST_MAX_STAGES + 16;
+    return sizeof(float) * ((size_t)N * KP4 + (size_t)ST_CWARPS * 2 * K * ST_PX + (size_t)ST_GROUPS * K * ST_PX) + 16 * ST_MAX_STAGES + 16;
 }
 inline int stages_of(int N, int K) {
     long long ns = ((long long)ST_SMEM_MAX - (long long)fixed_bytes_of(N, K)) / stage_bytes_of(N, K);
@@ -270,8 +295,8 @@ bool nmf_stream_available(const nmf_plan* p) { return p->st_ok; }
 
 size_t nmf_stream_workspace(const nmf_plan* p) {
     if (!p->st_ok) return 0;
-    const size_t one = (size_t)ctas_of(p, 1) * 2 * p->N * p->K * sizeof(float);
-    const size_t all = (size_t)p->batch * ctas_of(p, p->batch) * 2 * p->N * p->K * sizeof(float);
+    const size_t one = (size_t)ctas_of(p, 1) * ST_GROUPS * 2 * p->N * p->K * sizeof(float);
+    const size_t all = (size_t)p->batch * ctas_of(p, p->batch) * ST_GROUPS * 2 * p->N * p->K * sizeof(float);
     return one > all ? one : all;
 }
 
@@ -297,7 +322,7 @@ int nmf_stream_fit(nmf_plan* p, const float* X, const float* Om, float* W, float
                         K == 5 ? launch_stream<5>(a, grid, smem, p->stream, p->device) : K == 6 ? launch_stream<6>(a, grid, smem, p->stream, p->device) :
                         K == 7 ? launch_stream<7>(a, grid, smem, p->stream, p->device) : launch_stream<8>(a, grid, smem, p->stream, p->device);
         NMF_CUDA_TRY(p, e);
-        k_w_update_stream<<<dim3((nk + SU_E - 1) / SU_E, batch), SU_E * SU_Q, 0, p->stream>>>(a.slab, W, nk, ctas);
+        k_w_update_stream<<<dim3((nk + SU_E - 1) / SU_E, batch), SU_E * SU_Q, 0, p->stream>>>(a.slab, W, nk, ctas * ST_GROUPS);
         p->launches += 2;
         return NMF_OK;
     });
