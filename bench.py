@@ -313,6 +313,13 @@ def run_ours(args, rank, world, local_rank):
                     "tensor_time_floor_ms": F / (tpeak * 1e12) * 1e3,
                     "frac_of_sustained_peak": achieved / (bf16_s / 6.0),
                     "frac_of_ffma_roofline": achieved / ALU_PEAK_TFLOPS, "traffic_note": traffic_note, **roof_common}
+    elif plan.variant == 5:
+        # K <= 8: 12NKP flops are a fraction of the FP32 pipe; the kernel streams X and Omega once: HBM-bound
+        gbs = bytes_per_iter(N, P, K) / (fit_ms_avg * 1e-3) / 1e9
+        roofline = {"bound": "hbm", "achieved": gbs, "peak": hbm_peak, "unit": "GB/s", "frac": gbs / hbm_peak,
+                    "kernel": "fit iteration (k_stream: streaming FP32 kernel, K <= 8, + fixed-order reduce/W update)",
+                    "peak_source": "MEASURED_PEAKS.json hbm_gbs" if peaks else "fallback (B200_PROFILING.md)",
+                    "traffic_note": traffic_note, **roof_common}
     else:
         roofline = {"bound": "alu", "achieved": achieved, "peak": ALU_PEAK_TFLOPS, "unit": "TFLOP/s",
                     "frac": achieved / ALU_PEAK_TFLOPS,
@@ -328,7 +335,8 @@ def run_ours(args, rank, world, local_rank):
                    "step": "1 NMF iteration (a1-a8) + 1 projection iteration of M frames (a9) + subtraction (a10)",
                    "fit_variant": {1: "generic two-kernel", 2: "fused per-pixel-tile FFMA",
                                    3: "fused per-pixel-tile tcgen05 BF16x3",
-                                   4: "split tcgen05 BF16x3 (H half-step kernel + W half-step kernel)"}[plan.variant],
+                                   4: "split tcgen05 BF16x3 (H half-step kernel + W half-step kernel)",
+                                   5: "streaming FP32 kernel (K <= 8)"}[plan.variant],
                    "l2": "inputs (X+Omega 1.6 GB per step) are larger than the 126 MB L2; no explicit flush",
                    "parallelism": f"{world} independent replica(s), no collective"},
         "fit_ms_per_iter": fit_ms_avg,
@@ -454,7 +462,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="stis", choices=sorted(WORKLOADS))
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused FFMA, 3 tensor core")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core, 5 streaming FP32 (K <= 8)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=420.0,
                     help="--impl reference: seconds of oracle steps allowed at full size before falling back to a crop")

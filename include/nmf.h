@@ -41,7 +41,7 @@
  *     exactly into three BF16 pieces and six piece products per product, accumulated
  *     in fp32 (dropped terms <= 2^-22 relative, the level of a 3xTF32 split); the
  *     H update divides with the fast reciprocal (<= 2 ulp); sums across CTAs are
- *     fp64 in a fixed order.  The FFMA families (variants 1, 2) use plain fp32 FMA.
+ *     fp64 in a fixed order.  The FFMA families (variants 1, 2, 5) use plain fp32 FMA.
  *     Families therefore agree to fp32 rounding level, not bitwise.
  *   - A plan is bound to the CUDA device that was current when it was created;
  *     every call must be made with that device current (else INVALID_ARG).
@@ -60,7 +60,7 @@ typedef enum nmf_status {
     NMF_ERR_INVALID_ARG = -1, /* null pointer; N/P/K/M/iters out of range; M > max_targets   */
     NMF_ERR_ALIGNMENT   = -2, /* base pointer not 16-byte aligned or P % 4 != 0              */
     NMF_ERR_UNSUPPORTED = -3, /* N > 256, K > 128 or max_targets > 4096 (compiled limits); a
-                                 forced variant (2, 3, 4) whose kernels do not cover the shape */
+                                 forced variant (2 .. 5) whose kernels do not cover the shape */
     NMF_ERR_WORKSPACE   = -4, /* workspace missing or smaller than nmf_plan_workspace_bytes  */
     NMF_ERR_ARCH        = -5, /* current device is not compute capability 10.x               */
     NMF_ERR_CUDA        = -6, /* CUDA runtime / launch error (sticky until the plan is freed) */
@@ -95,18 +95,22 @@ int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
  *   0  automatic: the fastest family that covers the shape: the split tensor-core
  *      kernels (4) whenever K <= 128 and the operands fit shared memory, else the
  *      fused tensor-core kernel (3), else FFMA (2, 1); launch-bound problems of at most
- *      64 pixel tiles (128 px) in all run the fused FFMA kernel (2)
+ *      64 pixel tiles (128 px) in all run the fused FFMA kernel (2); K <= 8 runs the
+ *      streaming FP32 kernel (5)
  *   1  generic two-kernel FFMA path (any N <= 256, K <= 128; also what
  *      nmf_project runs when omega == NULL)
  *   2  fused FFMA per-pixel-tile kernel (K <= 50)
  *   3  fused tcgen05 kernel: one kernel per iteration does both half-steps (K <= 64)
  *   4  split tcgen05 kernels: H half-step kernel + W half-step kernel (K <= 128;
  *      N = 256 only up to K = 96)
- * A forced family (2, 3, 4) that does not cover the plan's shape makes the fit
+ *   5  streaming FP32 kernel: one kernel per iteration, X and Omega cross HBM once,
+ *      plain fp32 FMA, no BF16 split (K <= 8; fit only -- nmf_project of such a plan
+ *      runs family 4's projection kernel)
+ * A forced family (2, 3, 4, 5) that does not cover the plan's shape makes the fit
  * return UNSUPPORTED.  All families compute the updates of Eq. 3; see "Arithmetic"
- * above for how they differ.  Errors: INVALID_ARG (variant outside 0..4).          */
+ * above for how they differ.  Errors: INVALID_ARG (variant outside 0..5).          */
 int nmf_plan_set_variant(nmf_plan* plan, int variant);
-/* Which family (1..4) nmf_fit will run for this plan.                              */
+/* Which family (1..5) nmf_fit will run for this plan.                              */
 int nmf_plan_get_variant(const nmf_plan* plan);
 
 int nmf_plan_destroy(nmf_plan* plan); /* frees host state and any internal staging buffers */

@@ -58,7 +58,13 @@ k_stream(const __grid_constant__ StreamArgs g) {
     const int b = blockIdx.y;
     const float* __restrict__ Wg = g.W + (size_t)b * N * K;
     float* __restrict__ Hg = g.H + (size_t)b * K * g.P;
-    const uint32_t n_my = (uint32_t)((g.n_tiles - 1 - blockIdx.x) / gridDim.x) + 1u;    // gridDim.x <= n_tiles
+    // A CTA takes PAIRS of adjacent tiles (pair q = blockIdx.x + i gridDim.x, tiles 2q and 2q + 1, one per group): the two
+    // 128-byte segments of a row are requested close together in time.  gridDim.x <= number of pairs.
+    const long long n_pairs = (g.n_tiles + 1) / 2;
+    const uint32_t my_pairs = (uint32_t)((n_pairs - 1 - blockIdx.x) / gridDim.x) + 1u;
+    const bool last_half = (g.n_tiles & 1) && (blockIdx.x + (long long)(my_pairs - 1) * gridDim.x == n_pairs - 1);
+    const uint32_t n_my = 2u * my_pairs - (last_half ? 1u : 0u);
+    auto tile_px = [&](uint32_t i) -> long long { return ((blockIdx.x + (long long)(i >> 1) * gridDim.x) * 2 + (i & 1u)) * ST_PX; };
     const uint32_t NS = (uint32_t)g.NS;
 
     if (tid == 0) {
@@ -79,7 +85,7 @@ k_stream(const __grid_constant__ StreamArgs g) {
             for (uint32_t i = 0; i < n_my; ++i) {
                 const uint32_t s = i % NS, u = i / NS;
                 if (u > 0) mbar_wait(&empty[s], (u - 1u) & 1u);
-                const int p0 = (int)((blockIdx.x + (long long)i * gridDim.x) * ST_PX);
+                const int p0 = (int)tile_px(i);
                 const uint32_t dst = smem_u32(stages + (size_t)s * g.stage_bytes);
                 mbar_expect_tx(&full[s], tx_bytes);
                 tma_load_2d(dst, &g.mX, p0, b * N, &full[s]);
@@ -119,7 +125,7 @@ k_stream(const __grid_constant__ StreamArgs g) {
         const unsigned char* xs = stages + (size_t)s * g.stage_bytes;
         const unsigned char* os = xs + g.xbytes;
         const float* hs = reinterpret_cast<const float*>(xs + 2 * g.xbytes);      // [K][32]
-        const long long p0 = (blockIdx.x + (long long)it * gridDim.x) * ST_PX;
+        const long long p0 = tile_px(it);
         // ---------------- H half-step ----------------
         {
             float h[K], num[K], den[K];
@@ -261,11 +267,11 @@ inline int stages_of(int N, int K) {
     return ns > ST_MAX_STAGES ? ST_MAX_STAGES : ns < 0 ? 0 : (int)ns;
 }
 inline int ctas_of(const nmf_plan* p, int batch) {
-    const long long n_tiles = (p->P + ST_PX - 1) / ST_PX;
+    const long long n_tiles = ((p->P + ST_PX - 1) / ST_PX + 1) / 2;      // pairs of tiles
     long long avail = p->num_sms / batch;
     if (avail < 1) avail = 1;
     if (avail > n_tiles) avail = n_tiles;
-    const long long per = (n_tiles + avail - 1) / avail;      // every CTA gets `per` or `per - 1` tiles
+    const long long per = (n_tiles + avail - 1) / avail;      // every CTA gets `per` or `per - 1` pairs
     return (int)((n_tiles + per - 1) / per);
 }
 
