@@ -25,16 +25,47 @@ constexpr int ST_GROUPS = 2, ST_GWARPS = 8, ST_GTHREADS = 32 * ST_GWARPS;       
 constexpr int ST_CWARPS = ST_GROUPS * ST_GWARPS, ST_THREADS = 32 * (ST_CWARPS + 1), ST_PX = 32;   // + one TMA producer warp
 constexpr int ST_MAXK = 8;
 constexpr int ST_MAX_STAGES = 4;
+// iterations per call from which the tile-major copy of X, Omega pays: it costs about two iterations' time and saves 30 %
+// per iteration at K = 1 (HBM-bound), 13 % at K = 3, but only 1-3 % from K = 4 (issue-bound)
+inline int tiled_min_iters(int K) { return K <= 2 ? 8 : K == 3 ? 16 : 64; }
 constexpr size_t ST_SMEM_MAX = 227 * 1024;
 
 struct StreamArgs {
     CUtensorMap mX, mO;        // X, Om [B*N, P]: box [N frames][32 px], 128-byte swizzle
     CUtensorMap mH;            // H [B*K, P]: box [K][32 px]
     const float* W; float* H; float* slab;
+    const float* Xt; const float* Ot;   // tile-major copies of X and Omega (k_tile_major), or null: read X, Omega through mX, mO
     int N, NS; long long P; long long n_tiles;
     int xbytes;                // bytes of one X (or Omega) box, rounded up to 1024
     int stage_bytes;
 };
+
+// 1-D bulk copy global -> shared memory, completing on an mbarrier (bytes % 16 == 0, both addresses 16-byte aligned)
+__device__ __forceinline__ void bulk_load(uint32_t smem_dst, const void* src, uint32_t bytes, uint64_t* bar) {
+    asm volatile("cp.async.bulk.shared::cluster.global.mbarrier::complete_tx::bytes [%0], [%1], %2, [%3];"
+                 ::"r"(smem_dst), "l"(src), "r"(bytes), "r"(smem_u32(bar)) : "memory");
+}
+
+// Tile-major copy of X (z even) or Omega (z odd) of problem z / 2: out[tile][n][32 px] with the 16-byte chunks of a row
+// stored where the 128-byte swizzle puts them (chunk c of row n at c ^ (n & 7)), pixels beyond P as zeros -- byte for
+// byte the shared-memory image of a stage, so that a tile is ONE contiguous block of N x 128 bytes.
+// Why: with the caller's [N, P] layout every row of a tile is its own 128-byte request 4P bytes from the next (4 MB =
+// two pages at P = 1024^2) and the streaming kernel reached 4.4 TB/s; the same bytes with rows 256 KB apart (16 problems
+// of 65536 pixels) ran at 5.85 TB/s.  One pass of 2 x 8NP bytes per nmf_fit call, worth it from a few iterations up.
+__global__ void __launch_bounds__(256)
+k_tile_major(const float* __restrict__ X, const float* __restrict__ Om, float* __restrict__ Xt, float* __restrict__ Ot,
+             int N, long long P, long long n_tiles) {
+    const int n = blockIdx.y, b = blockIdx.z >> 1;
+    const float* __restrict__ src = ((blockIdx.z & 1) ? Om : X) + ((size_t)b * N + n) * P;
+    float* __restrict__ dst = ((blockIdx.z & 1) ? Ot : Xt) + (size_t)b * n_tiles * N * ST_PX;
+    const long long ch = (long long)blockIdx.x * 256 + threadIdx.x;      // 16-byte chunk of the row
+    if (ch >= n_tiles * 8) return;
+    const long long tile = ch >> 3;
+    const int c = (int)(ch & 7);
+    float4 v = make_float4(0.f, 0.f, 0.f, 0.f);
+    if (4 * ch < P) v = __ldg(reinterpret_cast<const float4*>(src + 4 * ch));     // P % 4 == 0
+    *reinterpret_cast<float4*>(dst + ((size_t)tile * N + n) * ST_PX + 4 * (c ^ (n & 7))) = v;
+}
 
 // Tiles alternate between the two groups (tile i of the CTA -> group i & 1), so that one group's H half-step overlaps
 // the other's W half-step; the stages form one ring filled by the producer warp.  An mbarrier wait tests a phase
@@ -88,8 +119,14 @@ k_stream(const __grid_constant__ StreamArgs g) {
                 const int p0 = (int)tile_px(i);
                 const uint32_t dst = smem_u32(stages + (size_t)s * g.stage_bytes);
                 mbar_expect_tx(&full[s], tx_bytes);
-                tma_load_2d(dst, &g.mX, p0, b * N, &full[s]);
-                tma_load_2d(dst + g.xbytes, &g.mO, p0, b * N, &full[s]);
+                if (g.Xt) {                              // tile-major copies: one contiguous block each
+                    const size_t off = ((size_t)b * g.n_tiles + (size_t)(p0 / ST_PX)) * N * ST_PX;
+                    bulk_load(dst, g.Xt + off, (uint32_t)N * 128u, &full[s]);
+                    bulk_load(dst + g.xbytes, g.Ot + off, (uint32_t)N * 128u, &full[s]);
+                } else {
+                    tma_load_2d(dst, &g.mX, p0, b * N, &full[s]);
+                    tma_load_2d(dst + g.xbytes, &g.mO, p0, b * N, &full[s]);
+                }
                 tma_load_2d(dst + 2 * g.xbytes, &g.mH, p0, b * K, &full[s]);
             }
         }
@@ -275,6 +312,16 @@ inline int ctas_of(const nmf_plan* p, int batch) {
     return (int)((n_tiles + per - 1) / per);
 }
 
+// workspace: slabs [batch][ctas][groups][2][N][K], then the tile-major copies of X and Omega (each batch x n_tiles x N x 32 floats)
+inline size_t slab_bytes_of(const nmf_plan* p) {
+    const size_t one = (size_t)ctas_of(p, 1) * ST_GROUPS * 2 * p->N * p->K * sizeof(float);
+    const size_t all = (size_t)p->batch * ctas_of(p, p->batch) * ST_GROUPS * 2 * p->N * p->K * sizeof(float);
+    return nmf_align_up(one > all ? one : all, 1024);
+}
+inline size_t tiled_bytes_of(const nmf_plan* p, int batch) {
+    return (size_t)batch * ((p->P + ST_PX - 1) / ST_PX) * p->N * ST_PX * sizeof(float);
+}
+
 template <int K>
 cudaError_t launch_stream(const StreamArgs& a, dim3 grid, size_t smem, cudaStream_t st, int device) {
     static bool done[NMF_MAX_DEVICES] = {};                   // the opt-in shared-memory size is a per-device attribute
@@ -301,9 +348,7 @@ bool nmf_stream_available(const nmf_plan* p) { return p->st_ok; }
 
 size_t nmf_stream_workspace(const nmf_plan* p) {
     if (!p->st_ok) return 0;
-    const size_t one = (size_t)ctas_of(p, 1) * ST_GROUPS * 2 * p->N * p->K * sizeof(float);
-    const size_t all = (size_t)p->batch * ctas_of(p, p->batch) * ST_GROUPS * 2 * p->N * p->K * sizeof(float);
-    return one > all ? one : all;
+    return slab_bytes_of(p) + 2 * tiled_bytes_of(p, p->batch);
 }
 
 int nmf_stream_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters, int batch) {
@@ -321,7 +366,18 @@ int nmf_stream_fit(nmf_plan* p, const float* X, const float* Om, float* W, float
     const int ctas = ctas_of(p, batch);
     const size_t smem = (size_t)a.NS * a.stage_bytes + fixed_bytes_of(N, K);
     const int nk = N * K;
-    int rc = nmf_run_iterations(p, 50, X, Om, W, H, nullptr, N, batch, iters, [&]() -> int {
+    // from tiled_min_iters(K) iterations per call X and Omega are first copied tile-major (k_tile_major says why)
+    const bool tiled = iters >= tiled_min_iters(K);
+    if (tiled) {
+        float* xt = reinterpret_cast<float*>(static_cast<char*>(p->ws) + slab_bytes_of(p));
+        float* ot = xt + tiled_bytes_of(p, batch) / sizeof(float);
+        const unsigned gx = (unsigned)((a.n_tiles * 8 + 255) / 256);
+        k_tile_major<<<dim3(gx, N, 2 * batch), 256, 0, p->stream>>>(X, Om, xt, ot, N, p->P, a.n_tiles);
+        p->launches++;
+        NMF_CUDA_TRY(p, cudaGetLastError());
+        a.Xt = xt; a.Ot = ot;
+    }
+    int rc = nmf_run_iterations(p, tiled ? 51 : 50, X, Om, W, H, nullptr, N, batch, iters, [&]() -> int {
         const dim3 grid(ctas, batch);
         cudaError_t e = K == 1 ? launch_stream<1>(a, grid, smem, p->stream, p->device) : K == 2 ? launch_stream<2>(a, grid, smem, p->stream, p->device) :
                         K == 3 ? launch_stream<3>(a, grid, smem, p->stream, p->device) : K == 4 ? launch_stream<4>(a, grid, smem, p->stream, p->device) :

@@ -101,7 +101,7 @@ def test_streaming_kernel_few_components(N, P, K, B):
     assert plan.variant == 5 or (P + 127) // 128 * B <= 64       # launch-bound sizes take the fused FFMA kernel
     plan = nmf.Plan(N, P, K, batch=B, variant=5)
     assert plan.variant == 5
-    iters = 9                                                     # graph replay of 9 (>= 8) iterations
+    iters = 9 if K <= 2 else 18 if K == 3 else 66                                  # enough for the tile-major copy (and a graph replay)
     res = []
     for garbage in (None, np.nan, 1e30):
         Xg = X.copy()
@@ -116,6 +116,15 @@ def test_streaming_kernel_few_components(N, P, K, B):
         res.append((Wd.cpu().numpy(), Hd.cpu().numpy()))
     for Wg, Hg in res[1:]:
         assert np.array_equal(Wg, res[0][0]) and np.array_equal(Hg, res[0][1])
+    # one call of `iters` iterations reads X and Omega from the tile-major copy, calls of 3 read the caller's arrays: same bits
+    Xd, Od, Wd, Hd = dev(X), dev(Om), dev(W0), dev(H0)
+    for _ in range(iters // 3):
+        if B == 1:
+            plan.fit(Xd[0], Od[0], Wd[0], Hd[0], 3)
+        else:
+            plan.fit_batched(Xd, Od, Wd, Hd, 3)
+    torch.cuda.synchronize()
+    assert np.array_equal(Wd.cpu().numpy(), res[0][0]) and np.array_equal(Hd.cpu().numpy(), res[0][1])
     Wg, Hg = res[0]
     for b in range(0, B, max(1, B // 4)):
         Wo, Ho = orc.fit(X[b], Om[b], W0[b], H0[b], iters)
