@@ -82,7 +82,8 @@ typedef struct nmf_plan nmf_plan; /* opaque; owns host-side launch state only */
 int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int max_targets);
 
 /* Bytes of device scratch the plan needs (split-K partial slabs, objective
- * partials).  The caller allocates it (16-byte aligned) and hands it over with
+ * partials; for K <= 8 also tile-major copies of X and Omega for the streaming
+ * kernel: 8 * N * P bytes per problem of the batch).  The caller allocates it (16-byte aligned) and hands it over with
  * nmf_plan_set_workspace; it must stay valid until the plan is destroyed or a
  * new workspace is set.  Contents need no initialisation.                      */
 size_t nmf_plan_workspace_bytes(const nmf_plan* plan);
