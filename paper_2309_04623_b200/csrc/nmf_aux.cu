@@ -13,9 +13,11 @@ constexpr int OBJ_THREADS = 128;
 
 // out[m,p] = t[m,p] - f[m] * sum_k c[m,k] H[k,p]; `fill` where omega[m,p] == 0.
 // Four pixels per thread (128-bit loads of H, T, omega; 128-bit stores), SUB_MC frames per launch handled as
-// SUB_MC / SUB_MH passes of SUB_MH frames: 64 accumulators keep the register count near 100, so five CTAs per SM
-// overlap one another's compute (K loop) and streaming (T, omega, out) phases; the H columns of the second pass
-// come back from L1 / L2.  Coefficients are 128-bit shared-memory broadcasts (cs[k][m]).
+// SUB_MC / SUB_MH groups of SUB_MH frames: 64 accumulators keep the register count near 100, so five CTAs per SM
+// overlap one another's compute (K loop) and streaming (T, omega, out) phases.  The frame groups of a pixel segment
+// are taken by ADJACENT CTAs (blockIdx.x = segment * groups + group): they run at the same time, so the H columns the
+// second one reads are in L2 (as two passes of one CTA they were 74 MB of other CTAs' traffic apart and missed: 1.3x
+// the algorithmic DRAM bytes).  Coefficients are 128-bit shared-memory broadcasts (cs[k][m]).
 __global__ void __launch_bounds__(SUB_THREADS, 5)
 k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float* __restrict__ C,
            const float* __restrict__ om, const float* __restrict__ factor, float fill,
@@ -27,9 +29,11 @@ k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float
         cs[i] = m < mc ? C[(size_t)(m0 + m) * K + k] : 0.f;
     }
     __syncthreads();
-    const long long p = ((long long)blockIdx.x * SUB_THREADS + threadIdx.x) * SUB_PX;
+    constexpr int NGRP = SUB_MC / SUB_MH;
+    const long long p = ((long long)(blockIdx.x / NGRP) * SUB_THREADS + threadIdx.x) * SUB_PX;
     if (p >= P) return;                            // P % 4 == 0: a segment is all in or all out
-    for (int mh = 0; mh < mc; mh += SUB_MH) {
+    const int mh = (int)(blockIdx.x % NGRP) * SUB_MH;
+    if (mh < mc) {
         float acc[SUB_MH][SUB_PX];
 #pragma unroll
         for (int m = 0; m < SUB_MH; ++m)
@@ -218,7 +222,7 @@ size_t nmf_aux_workspace(const nmf_plan* p) {
 int nmf_aux_subtract(nmf_plan* p, const float* H, const float* T, const float* C, const float* om,
                      const float* factor, float fill, float* out, int M) {
     const long long per_cta = (long long)SUB_THREADS * SUB_PX;
-    const unsigned grid = (unsigned)((p->P + per_cta - 1) / per_cta);
+    const unsigned grid = (unsigned)((p->P + per_cta - 1) / per_cta) * (SUB_MC / SUB_MH);
     const size_t smem = sizeof(float) * SUB_MC * p->K;
     for (int m0 = 0; m0 < M; m0 += SUB_MC) {
         k_subtract<<<grid, SUB_THREADS, smem, p->stream>>>(H, T, C, om, factor, fill, out, M, p->P, p->K, m0);
