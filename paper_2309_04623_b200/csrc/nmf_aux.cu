@@ -7,18 +7,19 @@ namespace {
 
 constexpr int SUB_MC = 32;      // science frames per pass (accumulators per thread)
 constexpr int SUB_THREADS = 128;
-constexpr int SUB_MH = 16;      // frames per register pass
+constexpr int SUB_MH = 8;       // frames per CTA (accumulator rows per thread)
 constexpr int SUB_PX = 4;       // pixels per thread (one 128-bit column segment of H, T, omega, out)
 constexpr int OBJ_THREADS = 128;
 
 // out[m,p] = t[m,p] - f[m] * sum_k c[m,k] H[k,p]; `fill` where omega[m,p] == 0.
 // Four pixels per thread (128-bit loads of H, T, omega; 128-bit stores), SUB_MC frames per launch handled as
-// SUB_MC / SUB_MH groups of SUB_MH frames: 64 accumulators keep the register count near 100, so five CTAs per SM
-// overlap one another's compute (K loop) and streaming (T, omega, out) phases.  The frame groups of a pixel segment
+// SUB_MC / SUB_MH groups of SUB_MH = 8 frames: 32 accumulators, 63 registers, eight CTAs per SM overlap one another's
+// compute (K loop) and streaming (T, omega, out) phases (16 frames per CTA: 0.169 ms, 8: 0.159 ms, 4: 0.37 ms -- the
+// coefficient loads and the 8-fold L2 read of H then dominate).  The frame groups of a pixel segment
 // are taken by ADJACENT CTAs (blockIdx.x = segment * groups + group): they run at the same time, so the H columns the
-// second one reads are in L2 (as two passes of one CTA they were 74 MB of other CTAs' traffic apart and missed: 1.3x
+// later ones read are in L2 (as two passes of one CTA they were 74 MB of other CTAs' traffic apart and missed: 1.3x
 // the algorithmic DRAM bytes).  Coefficients are 128-bit shared-memory broadcasts (cs[k][m]).
-__global__ void __launch_bounds__(SUB_THREADS, 5)
+__global__ void __launch_bounds__(SUB_THREADS, 8)
 k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float* __restrict__ C,
            const float* __restrict__ om, const float* __restrict__ factor, float fill,
            float* __restrict__ out, int M, long long P, int K, int m0) {
