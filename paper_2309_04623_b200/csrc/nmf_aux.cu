@@ -41,7 +41,7 @@ k_subtract(const float* __restrict__ H, const float* __restrict__ T, const float
 #pragma unroll
             for (int q = 0; q < SUB_PX; ++q) acc[m][q] = 0.f;
         const float* hp = H + p;
-        constexpr int KU = 5;                      // H rows in flight per thread
+        constexpr int KU = 5;                      // H rows in flight per thread (10: spills or fewer CTAs per SM, slower)
         for (int k0 = 0; k0 < K; k0 += KU) {
             float4 hv[KU];
 #pragma unroll
