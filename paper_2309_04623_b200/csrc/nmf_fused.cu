@@ -253,10 +253,10 @@ template <int KC>
 int launch(nmf_plan* p, const float* X, const float* Om, const float* W, float* H, int batch) {
     const int T = p->f_threads;
     const size_t smem = fused_smem(p->N, T, KC);
-    bool attr_done = false;   // function attributes are per device: set on every call (cheap)
-    if (!attr_done) {
+    static bool attr_done[NMF_MAX_DEVICES] = {};   // the opt-in shared-memory size is a per-device function attribute
+    if (!attr_done[p->device]) {
         NMF_CUDA_TRY(p, cudaFuncSetAttribute(k_fused_iter<KC>, cudaFuncAttributeMaxDynamicSharedMemorySize, 227 * 1024));
-        attr_done = true;
+        attr_done[p->device] = true;
     }
     const long long n_tiles = (p->P + T - 1) / T;
     dim3 grid(p->f_ctas, batch);
