@@ -17,7 +17,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 LIB = os.path.join(HERE, "libnmf_b200.so")
-SOURCES = ["nmf_api.cu", "nmf_generic.cu", "nmf_fused.cu", "nmf_tcfit.cu", "nmf_tcsplit.cu", "nmf_stream.cu", "nmf_aux.cu", "nmf_select.cu"]
+SOURCES = ["nmf_api.cu", "nmf_generic.cu", "nmf_fused.cu", "nmf_tcfit.cu", "nmf_tcsplit.cu", "nmf_stream.cu", "nmf_resident.cu", "nmf_aux.cu", "nmf_select.cu"]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 

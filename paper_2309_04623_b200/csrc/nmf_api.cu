@@ -15,6 +15,8 @@ size_t plan_workspace(nmf_plan* p) {
     if (ts > t) t = ts;
     size_t st = nmf_stream_workspace(p);
     if (st > t) t = st;
+    size_t rs = nmf_resident_workspace(p);
+    if (rs > t) t = rs;
     size_t sel = nmf_select_workspace(p);
     if (f > g) g = f;
     if (t > g) g = t;
@@ -44,6 +46,8 @@ int check_ws(const nmf_plan* p) {
 int pick_variant(const nmf_plan* p) {
     if (p->variant_req == 1) return 1;
     if (p->variant_req == 5) return nmf_stream_available(p) ? 5 : 1;
+    if (p->variant_req == 6) return nmf_resident_available(p) ? 6 : 1;
+    if (p->variant_req == 0 && nmf_resident_available(p)) return 6;    // small enough to stay on chip: one launch per fit
     if (p->variant_req == 2) return nmf_fused_available(p) ? 2 : 1;
     if (p->variant_req == 3) return nmf_tc_available(p) ? 3 : 1;
     if (p->variant_req == 0 && nmf_fused_available(p) && (p->P + 127) / 128 * p->batch <= 64) return 2;
@@ -66,7 +70,9 @@ int fit_common(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
     if (p->variant_req == 3 && !nmf_tc_available(p)) return NMF_ERR_UNSUPPORTED;
     if (p->variant_req == 4 && !nmf_tcsplit_available(p)) return NMF_ERR_UNSUPPORTED;
     if (p->variant_req == 5 && !nmf_stream_available(p)) return NMF_ERR_UNSUPPORTED;
+    if (p->variant_req == 6 && !nmf_resident_available(p)) return NMF_ERR_UNSUPPORTED;
     const int v = pick_variant(p);
+    if (v == 6) return nmf_resident_fit(p, X, Om, W, H, iters);
     if (v == 5) return nmf_stream_fit(p, X, Om, W, H, iters, batch);
     if (v == 4) return nmf_tcsplit_fit(p, X, Om, W, H, iters, batch);
     if (v == 3) return nmf_tc_fit(p, X, Om, W, H, iters, batch);
@@ -119,6 +125,7 @@ int nmf_plan_create(nmf_plan** out, int N, long long P, int K, int batch, int ma
     nmf_tc_configure(p);
     nmf_tcsplit_configure(p);
     nmf_stream_configure(p);
+    nmf_resident_configure(p);
     p->ws_needed = plan_workspace(p);
     *out = p;
     return NMF_OK;
@@ -160,7 +167,7 @@ int nmf_plan_set_stream(nmf_plan* p, void* s) {
 }
 
 int nmf_plan_set_variant(nmf_plan* p, int v) {
-    if (!p || v < 0 || v > 5) return NMF_ERR_INVALID_ARG;
+    if (!p || v < 0 || v > 6) return NMF_ERR_INVALID_ARG;
     p->variant_req = v;
     return NMF_OK;
 }
@@ -200,7 +207,7 @@ int nmf_project(nmf_plan* p, const float* H, const float* T, const float* om, fl
     if (iters == 0) return NMF_OK;
     // tensor-core W phase with H fixed when the plan's fit runs there too (omega == NULL: generic path)
     if (om && pick_variant(p) == 3) return nmf_tc_project(p, H, T, om, C, M, iters);
-    if (om && (pick_variant(p) == 4 || (pick_variant(p) == 5 && nmf_tcsplit_available(p))))   // (the streaming kernel is fit-only)
+    if (om && (pick_variant(p) == 4 || (pick_variant(p) >= 5 && nmf_tcsplit_available(p))))   // (families 5 and 6 are fit-only)
         return nmf_tcsplit_project(p, H, T, om, C, M, iters);
     return nmf_generic_project(p, H, T, om, C, M, iters);
 }

@@ -22,7 +22,7 @@ struct nmf_plan {
     void* ws = nullptr;
     size_t ws_bytes = 0;
     size_t ws_needed = 0;
-    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core, 5 streaming FP32
+    int variant_req = 0;          // 0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core, 5 streaming FP32, 6 resident
     long long launches = 0;
     int sticky = 0;               // first CUDA error seen (nmf_status)
     std::string cuda_msg;
@@ -42,6 +42,8 @@ struct nmf_plan {
     bool s_ok = false;
     // streaming FP32 kernel for K <= 8 (see nmf_stream.cu)
     bool st_ok = false;
+    // all iterations in one cooperative launch, problem resident on chip (see nmf_resident.cu)
+    bool rs_ok = false;
     // host staging for the *_host entry points (plan-owned device buffers)
     void* stage = nullptr;
     size_t stage_bytes = 0;
@@ -164,6 +166,11 @@ size_t nmf_stream_workspace(const nmf_plan* p);
 bool   nmf_stream_available(const nmf_plan* p);
 int    nmf_stream_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H,
                       int iters, int batch);
+// whole fit in one cooperative launch for problems that stay on chip: K <= 8, N <= 64, P <= 128 x SMs (nmf_resident.cu)
+void   nmf_resident_configure(nmf_plan* p);
+size_t nmf_resident_workspace(const nmf_plan* p);
+bool   nmf_resident_available(const nmf_plan* p);
+int    nmf_resident_fit(nmf_plan* p, const float* X, const float* Om, float* W, float* H, int iters);
 // closest-frame reference selection (nmf_select.cu)
 size_t nmf_select_workspace(const nmf_plan* p);
 int    nmf_select_distance(nmf_plan* p, const float* T, const float* ot, const float* X, const float* Om,

@@ -16,7 +16,7 @@ pytestmark = pytest.mark.gpu
 VARIANTS = [1, 2, 3, 4]   # generic, fused FFMA, fused tensor-core kernel (K <= 64), split tensor-core kernels (K <= 128; the automatic choice except for launch-bound sizes)
 
 
-@pytest.mark.parametrize("variant", VARIANTS + [5])    # 5 = streaming FP32 kernel, K <= 8
+@pytest.mark.parametrize("variant", VARIANTS + [5, 6])    # 5 = streaming FP32 kernel (K <= 8), 6 = resident kernel (one launch per fit)
 def test_tiny_full(variant):
     p = inputs.make_tiny()
     r = check_fit_parity(p, p.iters, variant)

@@ -47,7 +47,7 @@ def test_mask_invariance_bitwise(variant, garbage):
     assert torch.isfinite(out).all() and bool((out[dev(q.omega_t) == 0] == -1.0).all())
 
 
-@pytest.mark.parametrize("variant", VARIANTS + [5])
+@pytest.mark.parametrize("variant", VARIANTS + [5, 6])
 def test_power_of_two_homogeneity_bitwise(variant):
     p = inputs.make_tiny()
     W1, H1, plan = gpu_fit(p, 30, variant)
@@ -130,6 +130,41 @@ def test_streaming_kernel_few_components(N, P, K, B):
         Wo, Ho = orc.fit(X[b], Om[b], W0[b], H0[b], iters)
         assert rel(Wg[b], Wo) <= TOL_FACTOR and rel(Hg[b], Ho) <= TOL_FACTOR, (b, rel(Wg[b], Wo), rel(Hg[b], Ho))
         assert np.all(Hg[b][:, P // 2] == 0.0)
+
+
+@pytest.mark.parametrize("N,P,K", [(1, 4, 1), (3, 36, 2), (16, 4096, 5), (7, 132, 8), (64, 128 * 148, 3), (33, 128 * 147 + 20, 7)])
+def test_resident_kernel_small_problems(N, P, K):
+    """K <= 8, N <= 64, at most one 128-pixel tile per SM: the whole fit is ONE cooperative launch (variant 6; the automatic
+    choice there) with a grid-wide barrier per iteration: one CTA to all 148, ragged last tile, 1 + 40 + 41 iterations
+    against one call of 82 (bitwise), garbage where Omega == 0, oracle parity."""
+    rng = np.random.default_rng(N * 1000 + K)
+    X = (rng.random((N, P)) * 10).astype(np.float32)
+    Om = (rng.random((N, P)) * (rng.random((N, P)) > 0.25)).astype(np.float32)
+    Om[:, P // 2] = 0
+    W0 = (0.1 + 0.9 * rng.random((N, K))).astype(np.float32)
+    H0 = (0.1 + 0.9 * rng.random((K, P))).astype(np.float32)
+    plan = nmf.Plan(N, P, K)
+    assert plan.variant == 6
+    iters = 82
+    res = []
+    for garbage in (None, np.nan):
+        Xg = X.copy()
+        if garbage is not None:
+            Xg[Om == 0] = garbage
+        Xd, Od, Wd, Hd = dev(Xg), dev(Om), dev(W0), dev(H0)
+        plan.fit(Xd, Od, Wd, Hd, iters)
+        torch.cuda.synchronize()
+        res.append((Wd.cpu().numpy(), Hd.cpu().numpy()))
+    Xd, Od, Wd, Hd = dev(X), dev(Om), dev(W0), dev(H0)
+    for n in (1, 40, 41):
+        plan.fit(Xd, Od, Wd, Hd, n)
+    torch.cuda.synchronize()
+    res.append((Wd.cpu().numpy(), Hd.cpu().numpy()))
+    for Wg, Hg in res[1:]:
+        assert np.array_equal(Wg, res[0][0]) and np.array_equal(Hg, res[0][1])
+    Wo, Ho = orc.fit(X, Om, W0, H0, iters)
+    assert rel(res[0][0], Wo) <= TOL_FACTOR and rel(res[0][1], Ho) <= TOL_FACTOR, (rel(res[0][0], Wo), rel(res[0][1], Ho))
+    assert np.all(res[0][1][:, P // 2] == 0.0)
 
 
 def test_zero_entries_stay_zero_and_empty_iters():
@@ -339,11 +374,15 @@ def test_batched_more_problems_than_sms(variant):
 
 
 def test_automatic_family_selection():
-    """variant 0: the split tensor-core kernels wherever they fit, the fused FFMA kernel for launch-bound sizes (at most 64
-    pixel tiles in all), the generic kernels where nothing else covers the shape"""
+    """variant 0: the split tensor-core kernels wherever they fit, the streaming kernel for K <= 8, the resident kernel for
+    problems that stay on chip, the fused FFMA kernel for other launch-bound sizes (at most 64 pixel tiles in all), the
+    generic kernels where nothing else covers the shape"""
     assert nmf.Plan(200, 1 << 20, 50).variant == 4
     assert nmf.Plan(200, 1 << 20, 100).variant == 4
     assert nmf.Plan(128, 65536, 20, batch=64).variant == 4
-    assert nmf.Plan(16, 4096, 5).variant == 2
+    assert nmf.Plan(200, 1 << 20, 5).variant == 5
+    assert nmf.Plan(16, 4096, 5).variant == 6
+    assert nmf.Plan(16, 4096, 5, batch=2).variant == 2   # the resident kernel takes one problem
+    assert nmf.Plan(16, 4096, 12).variant == 2           # ... of at most 8 components
     assert nmf.Plan(16, 4096, 60).variant == 4          # no fused FFMA instantiation beyond K = 50
     assert nmf.Plan(256, 1 << 16, 128).variant == 1
