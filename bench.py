@@ -336,7 +336,8 @@ def run_ours(args, rank, world, local_rank):
                    "fit_variant": {1: "generic two-kernel", 2: "fused per-pixel-tile FFMA",
                                    3: "fused per-pixel-tile tcgen05 BF16x3",
                                    4: "split tcgen05 BF16x3 (H half-step kernel + W half-step kernel)",
-                                   5: "streaming FP32 kernel (K <= 8)"}[plan.variant],
+                                   5: "streaming FP32 kernel (K <= 8)",
+                                   6: "resident kernel (whole fit in one cooperative launch)"}[plan.variant],
                    "l2": "inputs (X+Omega 1.6 GB per step) are larger than the 126 MB L2; no explicit flush",
                    "parallelism": f"{world} independent replica(s), no collective"},
         "fit_ms_per_iter": fit_ms_avg,
@@ -462,7 +463,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default="stis", choices=sorted(WORKLOADS))
-    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core, 5 streaming FP32 (K <= 8)")
+    ap.add_argument("--variant", type=int, default=0, help="0 auto, 1 generic, 2 fused FFMA, 3 fused tensor core, 4 split tensor core, 5 streaming FP32 (K <= 8), 6 resident (small problems)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cpu-budget", type=float, default=420.0,
                     help="--impl reference: seconds of oracle steps allowed at full size before falling back to a crop")

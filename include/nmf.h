@@ -41,7 +41,7 @@
  *     exactly into three BF16 pieces and six piece products per product, accumulated
  *     in fp32 (dropped terms <= 2^-22 relative, the level of a 3xTF32 split); the
  *     H update divides with the fast reciprocal (<= 2 ulp); sums across CTAs are
- *     fp64 in a fixed order.  The FFMA families (variants 1, 2, 5) use plain fp32 FMA.
+ *     fp64 in a fixed order.  The FFMA families (variants 1, 2, 5, 6) use plain fp32 FMA.
  *     Families therefore agree to fp32 rounding level, not bitwise.
  *   - A plan is bound to the CUDA device that was current when it was created;
  *     every call must be made with that device current (else INVALID_ARG).
@@ -60,7 +60,7 @@ typedef enum nmf_status {
     NMF_ERR_INVALID_ARG = -1, /* null pointer; N/P/K/M/iters out of range; M > max_targets   */
     NMF_ERR_ALIGNMENT   = -2, /* base pointer not 16-byte aligned or P % 4 != 0              */
     NMF_ERR_UNSUPPORTED = -3, /* N > 256, K > 128 or max_targets > 4096 (compiled limits); a
-                                 forced variant (2 .. 5) whose kernels do not cover the shape */
+                                 forced variant (2 .. 6) whose kernels do not cover the shape */
     NMF_ERR_WORKSPACE   = -4, /* workspace missing or smaller than nmf_plan_workspace_bytes  */
     NMF_ERR_ARCH        = -5, /* current device is not compute capability 10.x               */
     NMF_ERR_CUDA        = -6, /* CUDA runtime / launch error (sticky until the plan is freed) */
@@ -97,7 +97,8 @@ int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
  *      kernels (4) whenever K <= 128 and the operands fit shared memory, else the
  *      fused tensor-core kernel (3), else FFMA (2, 1); launch-bound problems of at most
  *      64 pixel tiles (128 px) in all run the fused FFMA kernel (2); K <= 8 runs the
- *      streaming FP32 kernel (5)
+ *      streaming FP32 kernel (5); a single problem that stays on chip runs the
+ *      resident kernel (6)
  *   1  generic two-kernel FFMA path (any N <= 256, K <= 128; also what
  *      nmf_project runs when omega == NULL)
  *   2  fused FFMA per-pixel-tile kernel (K <= 50)
@@ -107,11 +108,14 @@ int nmf_plan_set_stream(nmf_plan* plan, void* cuda_stream);
  *   5  streaming FP32 kernel: one kernel per iteration, X and Omega cross HBM once,
  *      plain fp32 FMA, no BF16 split (K <= 8; fit only -- nmf_project of such a plan
  *      runs family 4's projection kernel)
- * A forced family (2, 3, 4, 5) that does not cover the plan's shape makes the fit
+ *   6  resident kernel: ALL iterations of a call in one cooperative launch, X, Omega
+ *      in shared memory and H in registers throughout, one grid-wide barrier per
+ *      iteration (K <= 8, N <= 64, P <= 128 x number of SMs, batch == 1; fit only)
+ * A forced family (2 .. 6) that does not cover the plan's shape makes the fit
  * return UNSUPPORTED.  All families compute the updates of Eq. 3; see "Arithmetic"
- * above for how they differ.  Errors: INVALID_ARG (variant outside 0..5).          */
+ * above for how they differ.  Errors: INVALID_ARG (variant outside 0..6).          */
 int nmf_plan_set_variant(nmf_plan* plan, int variant);
-/* Which family (1..5) nmf_fit will run for this plan.                              */
+/* Which family (1..6) nmf_fit will run for this plan.                              */
 int nmf_plan_get_variant(const nmf_plan* plan);
 
 int nmf_plan_destroy(nmf_plan* plan); /* frees host state and any internal staging buffers */
