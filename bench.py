@@ -374,7 +374,14 @@ def run_configs(args):
         H = torch.rand(shp(K, P), device="cuda") + 0.1
         fit = plan.fit_batched if B > 1 else plan.fit
         iters = max(3, min(200, int(2e11 / (12.0 * B * N * K * P))))
-        fit(X, Om, W, H, 3)
+        try:
+            fit(X, Om, W, H, 3)
+        except nmf.NMFError as e:                        # a forced family that does not cover this shape
+            print(f"[configs] {name}: variant {args.variant} unsupported ({e})", file=sys.stderr, flush=True)
+            out[name] = {"variant": args.variant, "unsupported": True}
+            del plan, X, Om, W, H
+            torch.cuda.empty_cache()
+            continue
         e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         torch.cuda.synchronize()
         e0.record(); fit(X, Om, W, H, iters); e1.record(); torch.cuda.synchronize()
